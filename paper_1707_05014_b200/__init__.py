@@ -1,0 +1,24 @@
+"""pct-b200: the hot path of proton-CT reconstruction (arxiv 1707.05014) as CUDA kernels for B200.
+
+The product is ``libpct.so`` (C ABI, ``include/pct.h``); this package is its thin ctypes binding
+with the same names.  Importing it requires the built CUDA library -- there is no CPU path.
+"""
+from ._build import build  # noqa: F401
+from .binding import (  # noqa: F401
+    EXPORTS,
+    FIELDS,
+    PctError,
+    lib,
+    pct_create,
+    pct_debug_block,
+    pct_debug_rows,
+    pct_destroy,
+    pct_get_image,
+    pct_get_stats,
+    pct_iterate,
+    pct_set_histories,
+    pct_set_histories_host,
+    pct_set_image,
+    pct_synchronize,
+    pct_version,
+)

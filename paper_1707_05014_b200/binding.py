@@ -1,0 +1,152 @@
+"""ctypes binding of libpct.so with the names of include/pct.h.
+
+Argument marshalling only: every step of the path (hull, MLP, voxel walk, DROP update) runs in the
+CUDA kernels of the library.  There is no CPU fallback: if the library cannot be built or loaded
+the import fails loudly.  torch appears only as the provider of device memory and streams
+(``tensor.data_ptr()``, ``torch.cuda.current_stream().cuda_stream``).
+"""
+import ctypes as C
+import os
+
+from . import _build
+
+PCT_OK, PCT_EINVAL, PCT_ENOMEM, PCT_ECUDA, PCT_ESTATE = 0, -1, -2, -3, -4
+_STATUS = {0: "PCT_OK", -1: "PCT_EINVAL", -2: "PCT_ENOMEM", -3: "PCT_ECUDA", -4: "PCT_ESTATE"}
+
+FIELDS = ("entry_t", "entry_v", "exit_t", "exit_v", "entry_dt", "entry_dv", "exit_dt", "exit_dv", "wepl")
+
+_FP = C.POINTER(C.c_float)
+_IP = C.POINTER(C.c_int32)
+
+
+class pct_histories(C.Structure):
+    _fields_ = [(n, C.c_void_p) for n in FIELDS] + [("proj", C.c_void_p), ("proj_cos", C.c_void_p),
+                                                     ("proj_sin", C.c_void_p), ("n_proj", C.c_int32)]
+
+
+class PctError(RuntimeError):
+    def __init__(self, code, msg):
+        super().__init__("%s: %s" % (_STATUS.get(code, code), msg))
+        self.code = code
+
+
+_lib = None
+
+
+def lib():
+    """Load (building first if needed) libpct.so.  Raises if that is impossible -- no fallback."""
+    global _lib
+    if _lib is None:
+        path = _build.LIB
+        if not os.path.exists(path) or os.environ.get("PCT_REBUILD"):
+            path = _build.build()
+        L = C.CDLL(path)
+        vp, i64 = C.c_void_p, C.c_int64
+        L.pct_create.argtypes = [C.POINTER(vp), C.c_int, C.c_int, C.c_int, C.c_float, C.c_float, C.c_float, vp]
+        L.pct_set_histories.argtypes = [vp, i64, C.POINTER(pct_histories)]
+        L.pct_set_histories_host.argtypes = [vp, i64, C.POINTER(pct_histories)]
+        L.pct_iterate.argtypes = [vp, C.c_float, i64, C.c_int]
+        L.pct_get_image.argtypes = [vp, vp, i64]
+        L.pct_set_image.argtypes = [vp, vp, i64]
+        L.pct_synchronize.argtypes = [vp]
+        L.pct_get_stats.argtypes = [vp, C.POINTER(i64)]
+        L.pct_destroy.argtypes = [vp]
+        L.pct_destroy.restype = None
+        L.pct_last_error.argtypes = [vp]
+        L.pct_last_error.restype = C.c_char_p
+        L.pct_version.restype = C.c_char_p
+        L.pct_debug_rows.argtypes = [vp, i64, i64, C.c_int32, vp, vp, vp, vp, vp, vp]
+        L.pct_debug_block.argtypes = [vp, i64, i64, vp, vp]
+        _lib = L
+    return _lib
+
+
+EXPORTS = ("pct_create", "pct_set_histories", "pct_set_histories_host", "pct_iterate", "pct_get_image",
+           "pct_set_image", "pct_synchronize", "pct_get_stats", "pct_destroy", "pct_last_error", "pct_version",
+           "pct_debug_rows", "pct_debug_block")
+
+
+def _ptr(a):
+    """Address of a torch tensor / numpy array / int / None."""
+    if a is None:
+        return None
+    if isinstance(a, int):
+        return a
+    if hasattr(a, "data_ptr"):
+        return a.data_ptr()
+    return a.ctypes.data
+
+
+def _check(ctx, rc):
+    if rc != PCT_OK:
+        raise PctError(rc, lib().pct_last_error(ctx).decode())
+
+
+def pct_version():
+    return lib().pct_version().decode()
+
+
+def pct_create(nx, ny, nz, voxel_mm, tracker_u_in_mm, tracker_u_out_mm, cuda_stream=None):
+    """-> opaque context handle (include/pct.h: pct_create)."""
+    h = C.c_void_p()
+    rc = lib().pct_create(C.byref(h), nx, ny, nz, voxel_mm, tracker_u_in_mm, tracker_u_out_mm, cuda_stream)
+    _check(None, rc)
+    return h
+
+
+def _hist_struct(arrays):
+    s = pct_histories()
+    keep = []
+    for k in FIELDS + ("proj", "proj_cos", "proj_sin"):
+        a = arrays[k]
+        keep.append(a)
+        setattr(s, k, _ptr(a))
+    s.n_proj = int(arrays["proj_cos"].shape[0])
+    return s, keep
+
+
+def pct_set_histories(ctx, n, arrays):
+    """arrays: mapping of CUDA tensors (float32 fields, uint16/int16 proj, float32 cos/sin tables), borrowed."""
+    s, _ = _hist_struct(arrays)
+    _check(ctx, lib().pct_set_histories(ctx, int(n), C.byref(s)))
+
+
+def pct_set_histories_host(ctx, n, arrays):
+    """arrays: mapping of host arrays (numpy or CPU tensors, ideally pinned); the library copies them."""
+    s, _ = _hist_struct(arrays)
+    _check(ctx, lib().pct_set_histories_host(ctx, int(n), C.byref(s)))
+
+
+def pct_iterate(ctx, lam, block_size, n_iter):
+    _check(ctx, lib().pct_iterate(ctx, float(lam), int(block_size), int(n_iter)))
+
+
+def pct_get_image(ctx, dst, n_voxels):
+    _check(ctx, lib().pct_get_image(ctx, _ptr(dst), int(n_voxels)))
+
+
+def pct_set_image(ctx, src, n_voxels):
+    _check(ctx, lib().pct_set_image(ctx, _ptr(src), int(n_voxels)))
+
+
+def pct_synchronize(ctx):
+    _check(ctx, lib().pct_synchronize(ctx))
+
+
+def pct_get_stats(ctx):
+    out = (C.c_int64 * 4)()
+    _check(ctx, lib().pct_get_stats(ctx, out))
+    return dict(rows=out[0], nnz=out[1], segments=out[2], histories=out[3])
+
+
+def pct_destroy(ctx):
+    lib().pct_destroy(ctx)
+
+
+def pct_debug_rows(ctx, first, count, max_seg, nseg, nnz, seg_idx=None, seg_len=None, row_len=None, nodes=None):
+    _check(ctx, lib().pct_debug_rows(ctx, int(first), int(count), int(max_seg), _ptr(nseg), _ptr(nnz), _ptr(seg_idx),
+                                     _ptr(seg_len), _ptr(row_len), _ptr(nodes)))
+
+
+def pct_debug_block(ctx, first, count, delta, cnt):
+    _check(ctx, lib().pct_debug_block(ctx, int(first), int(count), _ptr(delta), _ptr(cnt)))

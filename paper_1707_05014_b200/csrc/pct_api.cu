@@ -1,0 +1,377 @@
+// pct_api.cu -- the C ABI of include/pct.h: argument checks, device memory, the block loop.
+// No arithmetic of the path happens here except the host-side fp64 tables of step T / step G
+// of the rule, computed once per context.
+#include <math.h>
+#include <stdio.h>
+#include <stdlib.h>
+#include <string.h>
+
+#include <new>
+
+#include "../../include/pct.h"
+#include "pct_internal.h"
+
+using namespace pct;
+
+struct pct_ctx {
+    int device = 0;
+    cudaStream_t stream = nullptr;
+    Geom g{};
+    long long n_voxels = 0;
+    float* x = nullptr;
+    float2* acc = nullptr;
+    float4* tab = nullptr;
+    Ctrl* ctrl = nullptr;
+    int drop_grid = 0;
+    // histories
+    bool have_hist = false;
+    long long n = 0;
+    HistPtrs H{};
+    float* tables = nullptr;  // owned: pcos | psin
+    void* owned_hist = nullptr;  // owned device block of the host entry point
+    // cached CUDA graph of kGraphPairs (accumulate, update) pairs
+    cudaGraphExec_t graph = nullptr;
+    float graph_lambda = 0.f;
+    long long graph_block = 0, graph_n = 0;
+    const void* graph_hist_key = nullptr;
+    long long last_n_iter_hist = 0;
+    char err[512] = {0};
+};
+
+static thread_local char g_create_err[512] = {0};
+static const int kGraphPairs = 64;
+
+static int fail(pct_ctx* c, int code, const char* fmt, const char* detail = "") {
+    char* dst = c ? c->err : g_create_err;
+    snprintf(dst, 512, fmt, detail);
+    return code;
+}
+#define CUDA_TRY(c, call)                                                                  \
+    do {                                                                                   \
+        cudaError_t e__ = (call);                                                          \
+        if (e__ != cudaSuccess) {                                                          \
+            (void)cudaGetLastError();                                                      \
+            return fail((c), e__ == cudaErrorMemoryAllocation ? PCT_ENOMEM : PCT_ECUDA,    \
+                        #call ": %s", cudaGetErrorString(e__));                            \
+        }                                                                                  \
+    } while (0)
+
+// Rule step T: Sigma1^-1 at depth s = k*h, fp64 closed forms, rounded once to fp32.
+//   a_j = A_CM[j] * 0.1^j (j successive multiplications by 0.1) * 8192
+//   C = sum a_j s^(j+1)/(j+1), B = sum a_j s^(j+2)/((j+1)(j+2)), A = sum 2 a_j s^(j+3)/((j+1)(j+2)(j+3))
+//   W = (1 + 0.038 ln(s/361))^2 (A C - B^2);  (p11, p12, p22) = (C/W, -B/W, A/W)
+static void sigma1_inverse_table(float h32, int kmax, float4* out) {
+    static const double A_CM[6] = {7.457e-6, 4.548e-7, -5.777e-8, 1.301e-8, -9.228e-10, 2.687e-11};
+    double a[6];
+    for (int j = 0; j < 6; ++j) {
+        double v = A_CM[j];
+        for (int i = 0; i < j; ++i) v *= 0.1;
+        a[j] = v * 8192.0;
+    }
+    const double h = (double)h32;
+    out[0] = make_float4(0.f, 0.f, 0.f, 0.f);
+    for (int k = 1; k <= kmax; ++k) {
+        const double s = (double)k * h;
+        double A = 0.0, B = 0.0, C = 0.0, sp = s;
+        for (int j = 0; j < 6; ++j) {
+            C += a[j] * sp / (double)(j + 1);
+            B += a[j] * sp * s / (double)((j + 1) * (j + 2));
+            A += 2.0 * a[j] * sp * s * s / (double)((j + 1) * (j + 2) * (j + 3));
+            sp *= s;
+        }
+        const double gl = 1.0 + 0.038 * log(s / 361.0);
+        const double W = gl * gl * (A * C - B * B);
+        out[k] = make_float4((float)(C / W), (float)(-B / W), (float)(A / W), 0.f);
+    }
+}
+
+static void drop_graph(pct_ctx* c) {
+    if (c->graph) {
+        cudaGraphExecDestroy(c->graph);
+        c->graph = nullptr;
+    }
+}
+
+static void release_histories(pct_ctx* c) {
+    drop_graph(c);
+    if (c->owned_hist) cudaFree(c->owned_hist);
+    if (c->tables) cudaFree(c->tables);
+    c->owned_hist = nullptr;
+    c->tables = nullptr;
+    c->have_hist = false;
+    c->n = 0;
+}
+
+extern "C" const char* pct_version(void) { return "pct-b200 0.1 sm_100a"; }
+
+extern "C" const char* pct_last_error(const pct_ctx* ctx) { return ctx ? ctx->err : g_create_err; }
+
+extern "C" int pct_create(pct_ctx** out, int nx, int ny, int nz, float h, float u_in, float u_out, void* stream) {
+    if (!out) return fail(nullptr, PCT_EINVAL, "pct_create: out is NULL");
+    *out = nullptr;
+    if (nx < 1 || ny < 1 || nz < 1) return fail(nullptr, PCT_EINVAL, "pct_create: grid dimensions must be >= 1");
+    if ((long long)nx * ny * nz >= (1LL << 31)) return fail(nullptr, PCT_EINVAL, "pct_create: nx*ny*nz must be < 2^31");
+    if (!(h > 0.0f) || !isfinite(h)) return fail(nullptr, PCT_EINVAL, "pct_create: voxel_mm must be positive and finite");
+    const int nmin = nx < ny ? nx : ny;
+    if (nmin > 4096) return fail(nullptr, PCT_EINVAL, "pct_create: min(nx,ny) must be <= 4096");
+    // rule step G (fp32, this operation order)
+    Geom g{};
+    g.nx = nx; g.ny = ny; g.nz = nz; g.nmin = nmin;
+    g.h = h;
+    g.inv_h = 1.0f / h;
+    const float R = (0.5f * h) * (float)nmin;
+    g.R2 = R * R;
+    g.zmax = (0.5f * (float)nz) * h;
+    g.u_in = u_in; g.u_out = u_out;
+    g.hx = 0.5f * (float)nx; g.hy = 0.5f * (float)ny; g.hz = 0.5f * (float)nz;
+    if (!(u_in <= -R) || !(u_out >= R) || !isfinite(u_in) || !isfinite(u_out))
+        return fail(nullptr, PCT_EINVAL, "pct_create: tracker planes must lie outside the hull (u_in <= -R_h, u_out >= R_h)");
+    pct_ctx* c = new (std::nothrow) pct_ctx;
+    if (!c) return fail(nullptr, PCT_ENOMEM, "pct_create: out of host memory");
+    c->g = g;
+    c->n_voxels = (long long)nx * ny * nz;
+    c->stream = (cudaStream_t)stream;
+    int rc = PCT_OK;
+    auto body = [&]() -> int {
+        CUDA_TRY(nullptr, cudaGetDevice(&c->device));
+        CUDA_TRY(nullptr, cudaMalloc(&c->x, sizeof(float) * c->n_voxels));
+        CUDA_TRY(nullptr, cudaMalloc(&c->acc, sizeof(float2) * c->n_voxels));
+        CUDA_TRY(nullptr, cudaMalloc(&c->tab, sizeof(float4) * (nmin + 1)));
+        CUDA_TRY(nullptr, cudaMalloc(&c->ctrl, sizeof(Ctrl)));
+        CUDA_TRY(nullptr, cudaMemsetAsync(c->x, 0, sizeof(float) * c->n_voxels, c->stream));
+        CUDA_TRY(nullptr, cudaMemsetAsync(c->acc, 0, sizeof(float2) * c->n_voxels, c->stream));
+        CUDA_TRY(nullptr, cudaMemsetAsync(c->ctrl, 0, sizeof(Ctrl), c->stream));
+        float4* tab = (float4*)malloc(sizeof(float4) * (nmin + 1));
+        if (!tab) return fail(nullptr, PCT_ENOMEM, "pct_create: out of host memory");
+        sigma1_inverse_table(h, nmin, tab);
+        cudaError_t e = cudaMemcpyAsync(c->tab, tab, sizeof(float4) * (nmin + 1), cudaMemcpyHostToDevice, c->stream);
+        if (e == cudaSuccess) e = cudaStreamSynchronize(c->stream);
+        free(tab);
+        CUDA_TRY(nullptr, e);
+        CUDA_TRY(nullptr, drop_configure(nmin, &c->drop_grid));
+        return PCT_OK;
+    };
+    rc = body();
+    if (rc != PCT_OK) {
+        char keep[512];
+        memcpy(keep, g_create_err, 512);
+        pct_destroy(c);
+        memcpy(g_create_err, keep, 512);
+        return rc;
+    }
+    *out = c;
+    return PCT_OK;
+}
+
+extern "C" void pct_destroy(pct_ctx* c) {
+    if (!c) return;
+    cudaStreamSynchronize(c->stream);
+    release_histories(c);
+    if (c->x) cudaFree(c->x);
+    if (c->acc) cudaFree(c->acc);
+    if (c->tab) cudaFree(c->tab);
+    if (c->ctrl) cudaFree(c->ctrl);
+    (void)cudaGetLastError();
+    delete c;
+}
+
+static bool is_device_ptr(const void* p) {
+    cudaPointerAttributes at;
+    if (cudaPointerGetAttributes(&at, p) != cudaSuccess) {
+        (void)cudaGetLastError();
+        return false;
+    }
+    return at.type == cudaMemoryTypeDevice || at.type == cudaMemoryTypeManaged;
+}
+
+static int check_histories(pct_ctx* c, long long n, const pct_histories* h, bool want_device) {
+    if (!c) return PCT_EINVAL;
+    if (!h) return fail(c, PCT_EINVAL, "pct_set_histories: h is NULL");
+    if (n < 1 || n >= (1LL << 40)) return fail(c, PCT_EINVAL, "pct_set_histories: n must be in [1, 2^40)");
+    if (h->n_proj < 1 || h->n_proj > 65536) return fail(c, PCT_EINVAL, "pct_set_histories: n_proj must be in [1, 65536]");
+    const void* ptrs[12] = {h->entry_t, h->entry_v, h->exit_t, h->exit_v, h->entry_dt, h->entry_dv,
+                            h->exit_dt, h->exit_dv, h->wepl, h->proj, h->proj_cos, h->proj_sin};
+    for (int i = 0; i < 12; ++i) {
+        if (!ptrs[i]) return fail(c, PCT_EINVAL, "pct_set_histories: null array pointer");
+        if (is_device_ptr(ptrs[i]) != want_device)
+            return fail(c, PCT_EINVAL, want_device ? "pct_set_histories: arrays must be device memory"
+                                                   : "pct_set_histories_host: arrays must be host memory");
+    }
+    return PCT_OK;
+}
+
+extern "C" int pct_set_histories(pct_ctx* c, int64_t n, const pct_histories* h) {
+    int rc = check_histories(c, n, h, true);
+    if (rc) return rc;
+    release_histories(c);
+    CUDA_TRY(c, cudaMalloc(&c->tables, sizeof(float) * 2 * h->n_proj));
+    CUDA_TRY(c, cudaMemcpyAsync(c->tables, h->proj_cos, sizeof(float) * h->n_proj, cudaMemcpyDeviceToDevice, c->stream));
+    CUDA_TRY(c, cudaMemcpyAsync(c->tables + h->n_proj, h->proj_sin, sizeof(float) * h->n_proj, cudaMemcpyDeviceToDevice, c->stream));
+    c->H = HistPtrs{h->entry_t, h->entry_v, h->exit_t, h->exit_v, h->entry_dt, h->entry_dv, h->exit_dt, h->exit_dv,
+                    h->wepl, h->proj, c->tables, c->tables + h->n_proj, h->n_proj};
+    c->n = n;
+    c->have_hist = true;
+    return PCT_OK;
+}
+
+extern "C" int pct_set_histories_host(pct_ctx* c, int64_t n, const pct_histories* h) {
+    int rc = check_histories(c, n, h, false);
+    if (rc) return rc;
+    release_histories(c);
+    // one owned block: 9 float arrays (each padded to 256 B) + the uint16 array
+    const size_t fa = ((sizeof(float) * (size_t)n + 255) / 256) * 256;
+    const size_t total = 9 * fa + ((sizeof(uint16_t) * (size_t)n + 255) / 256) * 256;
+    CUDA_TRY(c, cudaMalloc(&c->owned_hist, total));
+    CUDA_TRY(c, cudaMalloc(&c->tables, sizeof(float) * 2 * h->n_proj));
+    const float* src[9] = {h->entry_t, h->entry_v, h->exit_t, h->exit_v, h->entry_dt, h->entry_dv, h->exit_dt, h->exit_dv, h->wepl};
+    const float* dst[9];
+    for (int i = 0; i < 9; ++i) {
+        float* d = (float*)((char*)c->owned_hist + i * fa);
+        dst[i] = d;
+        CUDA_TRY(c, cudaMemcpyAsync(d, src[i], sizeof(float) * (size_t)n, cudaMemcpyHostToDevice, c->stream));
+    }
+    uint16_t* dproj = (uint16_t*)((char*)c->owned_hist + 9 * fa);
+    CUDA_TRY(c, cudaMemcpyAsync(dproj, h->proj, sizeof(uint16_t) * (size_t)n, cudaMemcpyHostToDevice, c->stream));
+    CUDA_TRY(c, cudaMemcpyAsync(c->tables, h->proj_cos, sizeof(float) * h->n_proj, cudaMemcpyHostToDevice, c->stream));
+    CUDA_TRY(c, cudaMemcpyAsync(c->tables + h->n_proj, h->proj_sin, sizeof(float) * h->n_proj, cudaMemcpyHostToDevice, c->stream));
+    c->H = HistPtrs{dst[0], dst[1], dst[2], dst[3], dst[4], dst[5], dst[6], dst[7], dst[8], dproj,
+                    c->tables, c->tables + h->n_proj, h->n_proj};
+    c->n = n;
+    c->have_hist = true;
+    return PCT_OK;
+}
+
+static DropArgs drop_args(pct_ctx* c, long long block_size, long long first, long long count) {
+    DropArgs a{};
+    a.g = c->g;
+    a.H = c->H;
+    a.n = c->n;
+    a.block_size = block_size;
+    a.first = first;
+    a.count = count;
+    a.x = c->x;
+    a.acc = c->acc;
+    a.tab = c->tab;
+    a.ctrl = c->ctrl;
+    return a;
+}
+
+static int enqueue_pair(pct_ctx* c, const DropArgs& a, float lambda, long long n_blocks, cudaStream_t s) {
+    CUDA_TRY(c, launch_drop_block(a, c->drop_grid, s));
+    CUDA_TRY(c, launch_update(c->x, c->acc, c->n_voxels, lambda, c->ctrl, n_blocks, s));
+    return PCT_OK;
+}
+
+extern "C" int pct_iterate(pct_ctx* c, float lambda, int64_t block_size, int n_iter) {
+    if (!c) return PCT_EINVAL;
+    if (!c->have_hist) return fail(c, PCT_ESTATE, "pct_iterate: no histories set");
+    if (!(lambda > 0.0f) || !(lambda < 2.0f)) return fail(c, PCT_EINVAL, "pct_iterate: lambda must be in (0, 2)");
+    if (block_size < 1 || block_size > (1LL << 24)) return fail(c, PCT_EINVAL, "pct_iterate: block_size must be in [1, 2^24]");
+    if (n_iter < 0) return fail(c, PCT_EINVAL, "pct_iterate: n_iter must be >= 0");
+    if (n_iter == 0) return PCT_OK;
+    const long long n_blocks = (c->n + block_size - 1) / block_size;
+    const long long pairs = n_blocks * (long long)n_iter;
+    CUDA_TRY(c, cudaMemsetAsync(c->ctrl, 0, sizeof(Ctrl), c->stream));
+    const DropArgs a = drop_args(c, block_size, -1, 0);
+    long long done = 0;
+    if (pairs >= 2 * kGraphPairs) {
+        const bool reuse = c->graph && c->graph_lambda == lambda && c->graph_block == block_size && c->graph_n == c->n &&
+                           c->graph_hist_key == (const void*)c->H.t_in;
+        if (!reuse) {
+            drop_graph(c);
+            cudaStream_t cap = nullptr;
+            CUDA_TRY(c, cudaStreamCreateWithFlags(&cap, cudaStreamNonBlocking));
+            cudaGraph_t gr = nullptr;
+            int rc = PCT_OK;
+            cudaError_t e = cudaStreamBeginCapture(cap, cudaStreamCaptureModeThreadLocal);
+            if (e == cudaSuccess) {
+                for (int i = 0; i < kGraphPairs && rc == PCT_OK; ++i) rc = enqueue_pair(c, a, lambda, n_blocks, cap);
+                e = cudaStreamEndCapture(cap, &gr);
+            }
+            if (e == cudaSuccess && rc == PCT_OK) e = cudaGraphInstantiate(&c->graph, gr, 0);
+            if (gr) cudaGraphDestroy(gr);
+            cudaStreamDestroy(cap);
+            if (rc != PCT_OK) return rc;
+            CUDA_TRY(c, e);
+            c->graph_lambda = lambda;
+            c->graph_block = block_size;
+            c->graph_n = c->n;
+            c->graph_hist_key = (const void*)c->H.t_in;
+        }
+        for (; done + kGraphPairs <= pairs; done += kGraphPairs) CUDA_TRY(c, cudaGraphLaunch(c->graph, c->stream));
+    }
+    for (; done < pairs; ++done) {
+        int rc = enqueue_pair(c, a, lambda, n_blocks, c->stream);
+        if (rc) return rc;
+    }
+    return PCT_OK;
+}
+
+extern "C" int pct_synchronize(pct_ctx* c) {
+    if (!c) return PCT_EINVAL;
+    CUDA_TRY(c, cudaStreamSynchronize(c->stream));
+    return PCT_OK;
+}
+
+extern "C" int pct_get_image(pct_ctx* c, float* dst, int64_t n_voxels) {
+    if (!c) return PCT_EINVAL;
+    if (!dst || n_voxels != c->n_voxels) return fail(c, PCT_EINVAL, "pct_get_image: dst NULL or n_voxels != nx*ny*nz");
+    CUDA_TRY(c, cudaMemcpyAsync(dst, c->x, sizeof(float) * c->n_voxels, cudaMemcpyDefault, c->stream));
+    CUDA_TRY(c, cudaStreamSynchronize(c->stream));
+    return PCT_OK;
+}
+
+extern "C" int pct_set_image(pct_ctx* c, const float* src, int64_t n_voxels) {
+    if (!c) return PCT_EINVAL;
+    if (!src || n_voxels != c->n_voxels) return fail(c, PCT_EINVAL, "pct_set_image: src NULL or n_voxels != nx*ny*nz");
+    CUDA_TRY(c, cudaMemcpyAsync(c->x, src, sizeof(float) * c->n_voxels, cudaMemcpyDefault, c->stream));
+    if (!is_device_ptr(src)) CUDA_TRY(c, cudaStreamSynchronize(c->stream));
+    return PCT_OK;
+}
+
+extern "C" int pct_get_stats(pct_ctx* c, int64_t out[4]) {
+    if (!c || !out) return PCT_EINVAL;
+    Ctrl h;
+    CUDA_TRY(c, cudaMemcpyAsync(&h, c->ctrl, sizeof(Ctrl), cudaMemcpyDeviceToHost, c->stream));
+    CUDA_TRY(c, cudaStreamSynchronize(c->stream));
+    for (int i = 0; i < 3; ++i) out[i] = (int64_t)h.last[i];
+    out[3] = c->n;
+    return PCT_OK;
+}
+
+extern "C" int pct_debug_rows(pct_ctx* c, int64_t first, int64_t count, int32_t max_seg, int32_t* nseg, int32_t* nnz,
+                              int32_t* seg_idx, float* seg_len, float* row_len, float* nodes) {
+    if (!c) return PCT_EINVAL;
+    if (!c->have_hist) return fail(c, PCT_ESTATE, "pct_debug_rows: no histories set");
+    if (first < 0 || count < 1 || first + count > c->n) return fail(c, PCT_EINVAL, "pct_debug_rows: range outside the histories");
+    if (max_seg < c->g.nmin + 2) return fail(c, PCT_EINVAL, "pct_debug_rows: max_seg must be >= min(nx,ny)+2");
+    if (!nseg || !nnz) return fail(c, PCT_EINVAL, "pct_debug_rows: nseg and nnz are required");
+    const void* outs[6] = {nseg, nnz, seg_idx, seg_len, row_len, nodes};
+    for (int i = 0; i < 6; ++i)
+        if (outs[i] && !is_device_ptr(outs[i])) return fail(c, PCT_EINVAL, "pct_debug_rows: outputs must be device memory");
+    RowsArgs a{};
+    a.g = c->g;
+    a.H = c->H;
+    a.first = first;
+    a.count = count;
+    a.max_seg = max_seg;
+    a.tab = c->tab;
+    a.nseg = nseg; a.nnz = nnz; a.seg_idx = seg_idx;
+    a.seg_len = seg_len; a.row_len = row_len; a.nodes = nodes;
+    CUDA_TRY(c, launch_rows(a, c->stream));
+    return PCT_OK;
+}
+
+extern "C" int pct_debug_block(pct_ctx* c, int64_t first, int64_t count, float* delta, float* cnt) {
+    if (!c) return PCT_EINVAL;
+    if (!c->have_hist) return fail(c, PCT_ESTATE, "pct_debug_block: no histories set");
+    if (first < 0 || count < 1 || first + count > c->n) return fail(c, PCT_EINVAL, "pct_debug_block: range outside the histories");
+    if (!delta || !cnt || !is_device_ptr(delta) || !is_device_ptr(cnt))
+        return fail(c, PCT_EINVAL, "pct_debug_block: delta and cnt must be device memory");
+    CUDA_TRY(c, cudaMemsetAsync(c->ctrl, 0, sizeof(Ctrl), c->stream));
+    const DropArgs a = drop_args(c, count, first, count);
+    CUDA_TRY(c, launch_drop_block(a, c->drop_grid, c->stream));
+    CUDA_TRY(c, launch_split_acc(c->acc, delta, cnt, c->n_voxels, c->stream));
+    CUDA_TRY(c, cudaMemsetAsync(c->ctrl, 0, sizeof(Ctrl), c->stream));
+    return PCT_OK;
+}

@@ -1,0 +1,337 @@
+"""GPU parity: the CUDA path (through the C ABI) against the CPU oracle on the same seeded inputs.
+
+Bars (BASELINE.json north_star): voxel-index sequences bit-exact; MLP node positions within
+1e-4 mm of the fp64 definition; per-iteration image relative L2 error <= 1e-4; final RSP within
+1e-3 absolute per voxel.  Hit counts are integers: exact."""
+import numpy as np
+import pytest
+
+import synth
+from helpers import oracle_geom, slice_hist, to_device
+
+pytestmark = pytest.mark.gpu
+
+REL_L2_PER_ITER = 1e-4
+ABS_FINAL = 1e-3
+
+
+@pytest.fixture(scope="module")
+def torch_cuda():
+    import torch
+
+    assert torch.cuda.is_available(), "these tests need a CUDA device"
+    return torch
+
+
+@pytest.fixture(scope="module")
+def pct():
+    import paper_1707_05014_b200 as p
+
+    return p
+
+
+def _ctx(pct, torch, cfg):
+    return pct.pct_create(cfg.nx, cfg.ny, cfg.nz, cfg.h, cfg.u_in, cfg.u_out, torch.cuda.current_stream().cuda_stream)
+
+
+def _gpu_rows(pct, torch, ctx, first, count, nmin):
+    ms = nmin + 2
+    dev = "cuda"
+    nseg = torch.zeros(count, dtype=torch.int32, device=dev)
+    nnz = torch.zeros(count, dtype=torch.int32, device=dev)
+    seg_idx = torch.full((count, ms), -7, dtype=torch.int32, device=dev)
+    seg_len = torch.zeros((count, ms), dtype=torch.float32, device=dev)
+    row_len = torch.zeros((count, ms), dtype=torch.float32, device=dev)
+    nodes = torch.zeros((count, ms + 1, 3), dtype=torch.float32, device=dev)
+    pct.pct_debug_rows(ctx, first, count, ms, nseg, nnz, seg_idx, seg_len, row_len, nodes)
+    pct.pct_synchronize(ctx)
+    return [t.cpu().numpy() for t in (nseg, nnz, seg_idx, seg_len, row_len, nodes)]
+
+
+def _check_rows(oracle, pct, torch, cfg, H, stride=1, t64_every=7):
+    geom = oracle_geom(oracle, cfg)
+    hs = oracle.Histories(H)
+    D = to_device(H)
+    ctx = _ctx(pct, torch, cfg)
+    try:
+        pct.pct_set_histories(ctx, hs.n, D)
+        nseg, nnz, seg_idx, seg_len, row_len, nodes = _gpu_rows(pct, torch, ctx, 0, hs.n, geom.nmin)
+    finally:
+        pct.pct_destroy(ctx)
+    table = oracle.sigma1_table(geom.h, geom.nmin)
+    n_paths, worst64 = 0, 0.0
+    for i in range(0, hs.n, stride):
+        r = oracle.row_f32(geom, hs.hist(i), table)
+        ns = r["nseg"]
+        assert nseg[i] == ns, "history %d: segment count" % i
+        assert nnz[i] == r["nnz"], "history %d: nnz" % i
+        if ns == 0:
+            continue
+        n_paths += 1
+        # bit-exact: voxel index of every raw segment (the decision floor(fp32 midpoint))
+        assert np.array_equal(seg_idx[i, :ns], r["seg_idx"]), "history %d: voxel sequence" % i
+        # the whole rule is IEEE fp32 with a fixed operation order: lengths and nodes agree bitwise too
+        assert np.array_equal(seg_len[i, :ns], r["seg_len"]), "history %d: segment lengths" % i
+        assert np.array_equal(nodes[i, :ns + 1], r["nodes"]), "history %d: node positions" % i
+        # merged row: heads carry the merged length (fp32 sum in k order), others 0
+        heads = row_len[i, :ns] > 0
+        assert np.array_equal(seg_idx[i, :ns][heads], r["row_idx"])
+        assert row_len[i, :ns][heads] == pytest.approx(r["row_len"], rel=1e-6)
+        if (i // stride) % t64_every == 0:
+            n64, _ = oracle.path_f64(geom, hs.hist(i))
+            if n64 is not None and n64.shape[0] == ns + 1:
+                worst64 = max(worst64, float(np.abs(nodes[i, :ns + 1].astype(np.float64) - n64).max()))
+    assert worst64 < 1e-4  # MLP positions within 1e-4 mm of the fp64 matrix-form definition
+    return n_paths
+
+
+def test_rows_bit_exact_config0(oracle_mod, pct, torch_cuda):
+    cfg = synth.config(0)
+    H = synth.generate_numpy(cfg, 12000)
+    assert _check_rows(oracle_mod, pct, torch_cuda, cfg, H) > 8000
+
+
+@pytest.mark.parametrize("index,n,stride", [(1, 4000, 1), (2, 3000, 1), (3, 3000, 1), (4, 1500, 1)])
+def test_rows_bit_exact_larger_grids(oracle_mod, pct, torch_cuda, index, n, stride):
+    """Samples of the larger workloads: paths of 100-256 segments span 4-9 lane rounds and a ragged tail."""
+    cfg = synth.config(index)
+    H = synth.generate_numpy(cfg, n)
+    assert _check_rows(oracle_mod, pct, torch_cuda, cfg, H, stride) > n // 2
+
+
+def test_rows_bit_exact_odd_geometry(oracle_mod, pct, torch_cuda):
+    """Non-square grid, non-unit voxel (h = 0.8 mm), odd sizes: nmin = 45 -> hull radius 18 mm."""
+    base = synth.config(0)
+    cfg = synth.Config(9, "odd", 6000, 45, 71, 5, 0.8, 37, 500, 0.1, 1, base.shapes * 0.5, seed=99)
+    H = synth.generate_numpy(cfg, 6000)
+    assert _check_rows(oracle_mod, pct, torch_cuda, cfg, H) > 1500
+
+
+def test_rows_handcrafted_edge_cases(oracle_mod, pct, torch_cuda):
+    """Misses, grazing rays, NaN, paths leaving the grid in z (dropped segments break runs),
+    exactly axis-aligned central rays, steep rays."""
+    cfg = synth.config(0)
+    cs, sn = synth.generate.angle_table(cfg.n_angles)
+    rows = [
+        # t_in v_in t_out v_out tht_in thv_in tht_out thv_out proj
+        (0, 0, 0, 0, 0, 0, 0, 0, 0),            # central ray, axis aligned
+        (0, 0, 0, 0, 0, 0, 0, 0, 22),           # central ray, 88 degrees
+        (40, 0, 40, 0, 0, 0, 0, 0, 3),          # misses the hull
+        (31.9999, 0, 31.9999, 0, 0, 0, 0, 0, 5),  # grazing: L tiny
+        (32.0, 0, 32.0, 0, 0, 0, 0, 0, 5),      # tangent: disc == 0 -> skipped
+        (0, 4.5, 0, 0, 0, 0, 0, 0, 1),          # enters above the grid
+        (0, 3.9, 0, 3.9, 0, 0.02, 0, 0.02, 1),  # v rises: entry inside, exit hull point outside -> skipped
+        (0, 3.99, 0, -3.99, 0, -0.0831, 0, -0.0831, 7),  # steep in v, stays inside
+        (float("nan"), 0, 0, 0, 0, 0, 0, 0, 0),
+        (0, 0, float("inf"), 0, 0, 0, 0, 0, 0),
+        (5, 1, 9, -1, 0.05, -0.02, 0.03, -0.02, 11),  # large kink
+        (-20, -3.5, -22, 3.5, -0.02, 0.07, -0.02, 0.07, 45),
+        (10, 0, 10, 0, 0.3, 0, 0.3, 0, 17),     # 17 degree slope
+        (0, 0, 0.5, 0, 0, 0, 0, 0, 89),
+        (0, 3.19, 0, 3.19, 0, 0.05, 0, -0.05, 2),  # bulges above the grid: dropped segments split the row
+        (0, 3.73, 0, 3.73, 0, 0.01, 0, -0.01, 2),  # only the middle of the path is above the grid
+    ]
+    a = np.array(rows, dtype=np.float64)
+    H = dict(t_in=a[:, 0], v_in=a[:, 1], t_out=a[:, 2], v_out=a[:, 3], tht_in=a[:, 4], thv_in=a[:, 5],
+             tht_out=a[:, 6], thv_out=a[:, 7], wepl=np.ones(len(rows)), proj=a[:, 8].astype(np.uint16),
+             proj_cos=cs, proj_sin=sn)
+    H = {k: (v.astype(np.float32) if v.dtype == np.float64 else v) for k, v in H.items()}
+    n_paths = _check_rows(oracle_mod, pct, torch_cuda, cfg, H, t64_every=10 ** 9)
+    assert n_paths == 10
+
+
+def _block_parity(oracle, pct, torch, cfg, H, first, count, x0):
+    geom = oracle_geom(oracle, cfg)
+    hs = oracle.Histories(H)
+    D = to_device(H)
+    M = cfg.n_voxels
+    ctx = _ctx(pct, torch, cfg)
+    try:
+        pct.pct_set_histories(ctx, hs.n, D)
+        pct.pct_set_image(ctx, torch.from_numpy(x0.astype(np.float32)).cuda(), M)
+        delta = torch.zeros(M, dtype=torch.float32, device="cuda")
+        cnt = torch.zeros(M, dtype=torch.float32, device="cuda")
+        pct.pct_debug_block(ctx, first, count, delta, cnt)
+        pct.pct_synchronize(ctx)
+        # the accumulator must be left zeroed: a second call gives the same answer
+        delta2 = torch.zeros_like(delta)
+        cnt2 = torch.zeros_like(cnt)
+        pct.pct_debug_block(ctx, first, count, delta2, cnt2)
+        pct.pct_synchronize(ctx)
+    finally:
+        pct.pct_destroy(ctx)
+    d_ref, c_ref, stats = oracle.block_accumulate(geom, hs, first, count, x0.astype(np.float32).astype(np.float64))
+    assert np.array_equal(cnt.cpu().numpy(), c_ref.astype(np.float32))  # integers: exact
+    assert np.array_equal(cnt2.cpu().numpy(), c_ref.astype(np.float32))
+    d = delta.cpu().numpy().astype(np.float64)
+    scale = np.linalg.norm(d_ref)
+    assert np.linalg.norm(d - d_ref) <= 2e-5 * scale
+    assert np.abs(d - d_ref).max() <= 2e-4 * max(1.0, np.abs(d_ref).max())
+    assert np.linalg.norm(delta2.cpu().numpy() - d_ref) <= 2e-5 * scale
+    return stats
+
+
+def test_block_accumulate_from_zero_and_from_an_image(oracle_mod, pct, torch_cuda):
+    cfg = synth.config(0)
+    H = synth.generate_numpy(cfg, 9000)
+    st = _block_parity(oracle_mod, pct, torch_cuda, cfg, H, 0, 9000, np.zeros(cfg.n_voxels))
+    assert st[0] > 6000
+    x0 = synth.rsp_volume(cfg) * 0.9
+    _block_parity(oracle_mod, pct, torch_cuda, cfg, H, 1234, 4321, x0)  # ragged range, non-zero residuals near 10 %
+
+
+def test_block_accumulate_config2_sample(oracle_mod, pct, torch_cuda):
+    cfg = synth.config(2)
+    H = synth.generate_numpy(cfg, 20000)
+    x0 = synth.rsp_volume(cfg) * 0.8
+    _block_parity(oracle_mod, pct, torch_cuda, cfg, H, 0, 20000, x0)
+
+
+def _run_parity(oracle, pct, torch, cfg, H, lam, block, n_iter, x0=None, per_call=1):
+    """Full DROP run, image compared after every iteration."""
+    geom = oracle_geom(oracle, cfg)
+    hs = oracle.Histories(H)
+    D = to_device(H)
+    M = cfg.n_voxels
+    x_ref = np.zeros(M) if x0 is None else x0.astype(np.float32).astype(np.float64)
+    ctx = _ctx(pct, torch, cfg)
+    out = torch.zeros(M, dtype=torch.float32, device="cuda")
+    worst = 0.0
+    try:
+        pct.pct_set_histories(ctx, hs.n, D)
+        if x0 is not None:
+            pct.pct_set_image(ctx, x0.astype(np.float32), M)  # host pointer
+        for it in range(0, n_iter, per_call):
+            pct.pct_iterate(ctx, lam, block, per_call)
+            pct.pct_get_image(ctx, out, M)
+            x_ref, stats = oracle.drop_iterate(geom, hs, lam, block, per_call, x_ref)
+            x = out.cpu().numpy().astype(np.float64)
+            rel = np.linalg.norm(x - x_ref) / np.linalg.norm(x_ref)
+            worst = max(worst, rel)
+            assert rel <= REL_L2_PER_ITER, "iteration %d: rel L2 %.3g" % (it, rel)
+            gs = pct.pct_get_stats(ctx)
+            assert (gs["rows"], gs["nnz"]) == stats  # non-empty rows and non-zeros of the sweep: exact
+        assert np.abs(x - x_ref).max() <= ABS_FINAL
+    finally:
+        pct.pct_destroy(ctx)
+    return x, x_ref, worst
+
+
+def test_full_run_config0(oracle_mod, pct, torch_cuda):
+    """BASELINE.json configs[0] exactly: 1e5 protons, 64x64x8, B = 1e3, lambda = 0.1, 1 iteration."""
+    cfg = synth.config(0)
+    H = synth.generate_numpy(cfg)
+    x, x_ref, _ = _run_parity(oracle_mod, pct, torch_cuda, cfg, H, cfg.lam, cfg.block_size, cfg.n_iter)
+    assert np.linalg.norm(x_ref) > 1.0  # the image moved
+
+
+def test_config0_several_iterations_and_ragged_blocks(oracle_mod, pct, torch_cuda):
+    cfg = synth.config(0)
+    H = synth.generate_numpy(cfg, 30011)  # prime-ish: last block short (30011 = 42*700 + 611)
+    x, x_ref, _ = _run_parity(oracle_mod, pct, torch_cuda, cfg, H, 0.5, 700, 4)
+    # sanity: after 4 sweeps the water cylinder is near RSP 1 in the central slice
+    vol = x.reshape(cfg.nz, cfg.ny, cfg.nx)
+    assert 0.7 < vol[4, 32, 40] < 1.3
+
+
+def test_config1_sample(oracle_mod, pct, torch_cuda):
+    """configs[1] geometry and parameters on its first 4e5 histories (40 blocks of 1e4), 2 iterations."""
+    cfg = synth.config(1)
+    H = synth.generate_numpy(cfg, 400_000)
+    _run_parity(oracle_mod, pct, torch_cuda, cfg, H, cfg.lam, cfg.block_size, 2)
+
+
+def test_graph_path_and_call_splitting(oracle_mod, pct, torch_cuda):
+    """>= 128 (accumulate, update) pairs go through the replayed CUDA graph; one call with
+    n_iter = 3 equals three calls with n_iter = 1 (the image is the whole solver state)."""
+    cfg = synth.config(0)
+    H = synth.generate_numpy(cfg, 20000)
+    xa, ref_a, _ = _run_parity(oracle_mod, pct, torch_cuda, cfg, H, 0.3, 100, 3, per_call=3)   # 600 pairs in one call
+    xb, ref_b, _ = _run_parity(oracle_mod, pct, torch_cuda, cfg, H, 0.3, 100, 3, per_call=1)   # 200 pairs per call
+    assert np.array_equal(ref_a, ref_b)
+    assert np.linalg.norm(xa - xb) <= 1e-5 * np.linalg.norm(xa)
+
+
+def test_degenerate_inputs(oracle_mod, pct, torch_cuda):
+    torch = torch_cuda
+    cfg = synth.config(0)
+    H = synth.generate_numpy(cfg, 500)
+    # a single history, block larger than n
+    _run_parity(oracle_mod, pct, torch, cfg, slice_hist(H, slice(7, 8)), 1.0, 1000, 2)
+    # block size 1 (Kaczmarz order), lambda = 1
+    _run_parity(oracle_mod, pct, torch, cfg, slice_hist(H, slice(0, 60)), 1.0, 1, 1)
+    # every history misses the hull: the image stays at x0
+    Hm = {k: v.copy() for k, v in H.items()}
+    Hm["t_in"][:] = 45.0
+    Hm["t_out"][:] = 45.0
+    Hm["tht_in"][:] = 0
+    Hm["tht_out"][:] = 0
+    D = to_device(Hm)
+    ctx = _ctx(pct, torch, cfg)
+    try:
+        x0 = np.random.default_rng(0).uniform(0, 1, cfg.n_voxels).astype(np.float32)
+        pct.pct_set_histories(ctx, 500, D)
+        pct.pct_set_image(ctx, x0, cfg.n_voxels)
+        pct.pct_iterate(ctx, 0.5, 100, 2)
+        out = np.zeros(cfg.n_voxels, dtype=np.float32)
+        pct.pct_get_image(ctx, out, cfg.n_voxels)  # host destination
+        assert np.array_equal(out, x0)
+        assert pct.pct_get_stats(ctx)["rows"] == 0
+    finally:
+        pct.pct_destroy(ctx)
+
+
+def test_host_entry_point_matches_device_entry_point(oracle_mod, pct, torch_cuda):
+    from helpers import to_host_pct
+
+    torch = torch_cuda
+    cfg = synth.config(0)
+    H = synth.generate_numpy(cfg, 5000)
+    imgs = []
+    for host in (False, True):
+        ctx = _ctx(pct, torch, cfg)
+        try:
+            if host:
+                pct.pct_set_histories_host(ctx, 5000, to_host_pct(H))
+            else:
+                D = to_device(H)
+                pct.pct_set_histories(ctx, 5000, D)
+            pct.pct_iterate(ctx, 0.2, 500, 2)
+            out = np.zeros(cfg.n_voxels, dtype=np.float32)
+            pct.pct_get_image(ctx, out, cfg.n_voxels)
+            imgs.append(out)
+        finally:
+            pct.pct_destroy(ctx)
+    assert np.linalg.norm(imgs[0] - imgs[1]) <= 1e-5 * np.linalg.norm(imgs[0])
+
+
+def test_error_reporting(pct, torch_cuda):
+    torch = torch_cuda
+    cfg = synth.config(0)
+    ctx = _ctx(pct, torch, cfg)
+    try:
+        with pytest.raises(pct.PctError) as e:
+            pct.pct_iterate(ctx, 0.1, 10, 1)
+        assert e.value.code == -4  # PCT_ESTATE: no histories yet
+        H = synth.generate_numpy(cfg, 100)
+        D = to_device(H)
+        with pytest.raises(pct.PctError) as e:
+            pct.pct_set_histories(ctx, 0, D)
+        assert e.value.code == -1
+        from helpers import to_host_pct
+
+        with pytest.raises(pct.PctError) as e:
+            pct.pct_set_histories(ctx, 100, to_host_pct(H))  # host pointers where device is required
+        assert e.value.code == -1
+        pct.pct_set_histories(ctx, 100, D)
+        for lam, b, it in [(0.0, 10, 1), (2.0, 10, 1), (0.1, 0, 1), (0.1, 10, -1), (0.1, 2 ** 24 + 1, 1), (float("nan"), 10, 1)]:
+            with pytest.raises(pct.PctError) as e:
+                pct.pct_iterate(ctx, lam, b, it)
+            assert e.value.code == -1
+        with pytest.raises(pct.PctError):
+            pct.pct_get_image(ctx, torch.zeros(10, device="cuda"), 10)
+        pct.pct_iterate(ctx, 0.1, 10, 0)  # zero iterations: a no-op
+        pct.pct_iterate(ctx, 0.1, 10, 1)
+        pct.pct_synchronize(ctx)
+    finally:
+        pct.pct_destroy(ctx)

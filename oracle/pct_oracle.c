@@ -334,6 +334,18 @@ typedef struct {
     int K;
 } r32_state;
 
+/* c + cl = t_pl - theta*u_pl to about twice fp32 precision: p + pe = theta*u_pl exactly (fma),
+ * c + e = t_pl - p exactly (two-sum), cl = e - pe. */
+static void r32_ray_offset(float t_pl, float theta, float u_pl, float *c_out, float *cl_out) {
+    const float p = theta * u_pl;
+    const float pe = fmaf(theta, u_pl, -p);
+    const float c = t_pl - p;
+    const float bb = c - t_pl;
+    const float e = (t_pl - (c - bb)) + (-p - bb);
+    *c_out = c;
+    *cl_out = e - pe;
+}
+
 /* hull + per-history set-up.  Returns 1 if the history has a path, 0 if skipped (R7). */
 static int r32_setup(const orc_geom *g, const orc_hist *hh, r32_state *st) {
     const float h = g->h;
@@ -342,13 +354,16 @@ static int r32_setup(const orc_geom *g, const orc_hist *hh, r32_state *st) {
     const float R = (0.5f * h) * (float)nmin;
     const float R2 = R * R;
     const float zmax = (0.5f * (float)g->nz) * h;
-    /* step 1 */
+    /* step 1: ray t = c + theta*u with c = t_pl - theta*u_pl carried as c + cl (product and sum
+     * errors recovered exactly), discriminant R^2(1+theta^2) - c^2 = (R-c)(R+c) + R^2 theta^2:
+     * no cancellation of rounded squares, so grazing rays keep their hull points to ~1e-5 mm */
+    float c_in, cl_in, c_out, cl_out;
+    r32_ray_offset(hh->t_in, hh->tht_in, g->u_in, &c_in, &cl_in);
+    r32_ray_offset(hh->t_out, hh->tht_out, g->u_out, &c_out, &cl_out);
     const float q_in = fmaf(hh->tht_in, hh->tht_in, 1.0f);
-    const float c_in = fmaf(-hh->tht_in, g->u_in, hh->t_in);
-    const float disc_in = fmaf(R2, q_in, -(c_in * c_in));
     const float q_out = fmaf(hh->tht_out, hh->tht_out, 1.0f);
-    const float c_out = fmaf(-hh->tht_out, g->u_out, hh->t_out);
-    const float disc_out = fmaf(R2, q_out, -(c_out * c_out));
+    const float disc_in = fmaf((R - c_in) - cl_in, (R + c_in) + cl_in, R2 * (hh->tht_in * hh->tht_in));
+    const float disc_out = fmaf((R - c_out) - cl_out, (R + c_out) + cl_out, R2 * (hh->tht_out * hh->tht_out));
     if (!(disc_in > 0.0f) || !(disc_out > 0.0f)) return 0;
     const float u0 = fmaf(-hh->tht_in, c_in, -sqrtf(disc_in)) / q_in;
     const float u2 = fmaf(-hh->tht_out, c_out, sqrtf(disc_out)) / q_out;

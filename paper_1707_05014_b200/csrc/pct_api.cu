@@ -120,6 +120,7 @@ extern "C" int pct_create(pct_ctx** out, int nx, int ny, int nz, float h, float 
     g.h = h;
     g.inv_h = 1.0f / h;
     const float R = (0.5f * h) * (float)nmin;
+    g.R = R;
     g.R2 = R * R;
     g.zmax = (0.5f * (float)nz) * h;
     g.u_in = u_in; g.u_out = u_out;

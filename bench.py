@@ -1,0 +1,365 @@
+#!/usr/bin/env python
+"""bench.py -- protons*iterations/s of the pCT hot path (MLP + voxel walk + DROP projection) on B200.
+
+Contract (driver): ``python bench.py --gpus N --steps K --warmup W`` prints ONE JSON line on rank 0.
+  * workload: BASELINE.json configs[3] (5e8 synthetic protons, 256x256x128 grid, B = 1e5, lambda = 0.05),
+    the configuration the metric is quoted on; it fits one GPU (19 GB of histories).
+  * a "step" = ONE DROP sweep over all N histories (rows a0-a6 of SURVEY.md section 8(a): history
+    stream, hull, MLP, voxel walk, row projection, scatter, block update; 5000 blocks), i.e. one
+    iteration of the paper's solver; `value` = N / step time = protons*iterations/s.
+  * `value`: histories resident in HBM; `e2e`: the same step through the C ABI from pinned HOST
+    arrays (pct_set_histories_host -> pct_iterate -> pct_get_image to host), copies inside the timing.
+  * `roofline`: the fused accumulate kernel, timed with CUDA events around every launch
+    (pct_profile_sweep); `cpu_baseline`: the oracle timed on this box's host cores on a bounded sample.
+  * ``--impl reference``: the oracle as it stands on the host cores (there is no reference code).
+  * N > 1 (torchrun): replicas only -- every rank runs the same workload on its own histories, no
+    data-path collective; value = sum of histories / max time.
+Inputs are seeded synthetic histories (synth/), generated on the GPU; nothing reads /root/reference.
+"""
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+METRIC = "protons*iterations/s (MLP+projection)"
+UNIT = "protons*iterations/s"
+
+# Algorithmic work per unit, derived in DESIGN.md "Roofline": per raw path segment the rule
+# prescribes 106 fp32/int operations (70 MLP node + 30 segment/voxel + 6 projection, FMA = 1);
+# per history 38 B of HBM; per segment one 4 B gather, per non-zero one 8 B (Delta, c) reduction.
+OPS_PER_SEGMENT = 106
+HBM_BYTES_PER_HISTORY = 38
+SM_COUNT = 148
+LANES_PER_SM = 128
+
+
+def parse_args():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=5)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--config", type=int, default=3, help="BASELINE.json configs index (default 3, the metric's)")
+    ap.add_argument("--histories", type=float, default=None, help="override N (debugging only; reported)")
+    ap.add_argument("--e2e-steps", type=int, default=2)
+    ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--no-cpu", action="store_true")
+    ap.add_argument("--cpu-seconds", type=float, default=15.0, help="target CPU time of the oracle sample")
+    return ap.parse_args()
+
+
+def measured_peaks():
+    try:
+        with open(os.path.join(ROOT, "MEASURED_PEAKS.json")) as f:
+            p = json.load(f)
+        return dict(hbm_gbs=float(p["hbm_gbs"]), sm_max_mhz=float(p.get("sm_max_mhz", 1965.0)), source="measured")
+    except (OSError, KeyError, ValueError):
+        return dict(hbm_gbs=6650.0, sm_max_mhz=1965.0, source="fallback")
+
+
+class ClockSampler:
+    """nvidia-smi clocks and throttle reasons sampled every 200 ms while the timed region runs."""
+
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
+         "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index):
+        self.index = index
+        self.lines = []
+        self.proc = None
+
+    def __enter__(self):
+        try:
+            self.proc = subprocess.Popen(["nvidia-smi", "-i", str(self.index), "--query-gpu=" + self.Q,
+                                          "--format=csv,noheader,nounits", "-lms", "200"],
+                                         stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            self.thread = threading.Thread(target=self._read, daemon=True)
+            self.thread.start()
+        except OSError:
+            self.proc = None
+        return self
+
+    def _read(self):
+        for line in self.proc.stdout:
+            self.lines.append(line.strip())
+
+    def __exit__(self, *exc):
+        if self.proc is not None:
+            self.proc.terminate()
+            try:
+                self.proc.wait(timeout=5)
+            except subprocess.TimeoutExpired:
+                self.proc.kill()
+            self.thread.join(timeout=2)
+
+    def summary(self):
+        sm, mx, pw, reasons = [], [], [], set()
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for ln in self.lines:
+            f = [s.strip() for s in ln.split(",")]
+            if len(f) < 7:
+                continue
+            try:
+                sm.append(float(f[0])); mx.append(float(f[1])); pw.append(float(f[2]))
+            except ValueError:
+                continue
+            for name, val in zip(names, f[3:7]):
+                if val.lower().startswith("active"):
+                    reasons.add(name)
+        if not sm:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": [], "samples": 0}
+        sm.sort()
+        return {"sm_mhz": sm[len(sm) // 2], "sm_max_mhz": max(mx), "power_w_max": max(pw), "reasons": sorted(reasons),
+                "samples": len(sm)}
+
+
+def cpu_oracle_rate(cfg, H, target_seconds, max_blocks=64):
+    """The oracle as it stands (oracle/, OpenMP over the histories of a block) on the host cores:
+    DROP sweep from x0 = 0 over the first blocks of the workload.  -> (rate, cores, blocks, seconds)."""
+    import numpy as np
+
+    import oracle
+
+    oracle.build()
+    geom = oracle.Geometry(cfg.nx, cfg.ny, cfg.nz, cfg.h, cfg.u_in, cfg.u_out)
+    hs = oracle.Histories(H)
+    B = cfg.block_size
+    avail = hs.n // B
+    t0 = time.perf_counter()
+    oracle.drop_iterate(geom, hs, cfg.lam, B, 1, np.zeros(cfg.n_voxels), n=B)
+    t1 = time.perf_counter() - t0
+    nb = int(max(1, min(avail, max_blocks, round(target_seconds / max(t1, 1e-3)))))
+    t0 = time.perf_counter()
+    oracle.drop_iterate(geom, hs, cfg.lam, B, 1, np.zeros(cfg.n_voxels), n=nb * B)
+    dt = time.perf_counter() - t0
+    return nb * B / dt, oracle.num_threads(), nb, dt
+
+
+def run_reference(args):
+    """--impl reference: there is no reference code (the paper ships none); the arm is the oracle,
+    unmodified, on the host cores.  A step = one DROP sweep over a bounded sample of the workload."""
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    import numpy as np
+
+    import oracle
+    import synth
+
+    cfg = synth.config(args.config)
+    B = cfg.block_size
+    nb = 4  # blocks per step: 4e5 histories of configs[3]
+    H = synth.generate_numpy(cfg, nb * B)
+    oracle.build()
+    geom = oracle.Geometry(cfg.nx, cfg.ny, cfg.nz, cfg.h, cfg.u_in, cfg.u_out)
+    hs = oracle.Histories(H)
+    x = np.zeros(cfg.n_voxels)
+    for _ in range(args.warmup):
+        oracle.drop_iterate(geom, hs, cfg.lam, B, 1, x)
+    t0 = time.perf_counter()
+    for _ in range(args.steps):
+        oracle.drop_iterate(geom, hs, cfg.lam, B, 1, x)
+    dt = time.perf_counter() - t0
+    rate = nb * B * args.steps / dt
+    cores = oracle.num_threads()
+    sample = "%d blocks of %d histories of %s per step (generated by synth.generate_numpy)" % (nb, B, cfg.workload)
+    print(json.dumps({
+        "impl": "reference", "metric": METRIC, "value": rate, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
+        "warmup": args.warmup, "ms_per_step": dt / args.steps * 1e3, "higher_is_better": True, "scaling": "weak",
+        "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+        "config": {"workload": cfg.workload, "grid": [cfg.nx, cfg.ny, cfg.nz], "block_size": B, "lambda": cfg.lam,
+                   "histories_per_step": nb * B, "note": "CPU oracle (fp64 accumulation, fp32 rule rows); bounded sample"},
+        "cpu_baseline": {"value": rate, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample},
+        "e2e": {"value": rate, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "gpu_launches": 0,
+    }))
+
+
+def run_ours(args):
+    import numpy as np
+    import torch
+    import torch.distributed as dist
+
+    import paper_1707_05014_b200 as pct  # fails loudly if libpct.so cannot be built/loaded: no CPU path
+    import synth
+    import synth.cuda_gen as cuda_gen
+
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    assert torch.cuda.is_available(), "bench.py needs a CUDA device: the path has no CPU fallback"
+    torch.cuda.set_device(local)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+
+    def max_over_ranks(v):
+        if world == 1:
+            return v
+        t = torch.tensor([v], dtype=torch.float64, device="cuda")
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        return float(t.item())
+
+    cfg = synth.config(args.config)
+    n = cfg.n if args.histories is None else int(args.histories)
+    B, lam, M = cfg.block_size, cfg.lam, cfg.n_voxels
+    n_blocks = (n + B - 1) // B
+
+    # replicas only: rank r draws histories [r*n, (r+1)*n) of the same seeded stream
+    D = cuda_gen.generate_cuda(cfg, n, first=rank * n)
+    P = synth.to_pct_names(D)
+    stream = torch.cuda.Stream()
+    out = {}
+    with torch.cuda.stream(stream):  # torch.cuda.Event records on this stream, the one the kernels run on
+        ctx = pct.pct_create(cfg.nx, cfg.ny, cfg.nz, cfg.h, cfg.u_in, cfg.u_out, stream.cuda_stream)
+        try:
+            pct.pct_set_histories(ctx, n, P)
+            for _ in range(args.warmup):
+                pct.pct_iterate(ctx, lam, B, 1)
+            pct.pct_synchronize(ctx)
+            barrier()
+            torch.cuda.synchronize()
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            with ClockSampler(local) as clk:
+                e0.record()
+                for _ in range(args.steps):
+                    pct.pct_iterate(ctx, lam, B, 1)
+                e1.record()
+                torch.cuda.synchronize()
+                barrier()
+            ms = max_over_ranks(e0.elapsed_time(e1))
+            out["ms_per_step"] = ms / args.steps
+            out["value"] = world * n * args.steps / (ms * 1e-3)
+            out["clocks"] = clk.summary()
+            out["stats"] = pct.pct_get_stats(ctx)
+            # the dominant kernel, CUDA events around every launch, one more sweep of the same workload
+            prof = pct.pct_profile_sweep(ctx, lam, B)
+            out["prof"] = prof
+            img = torch.empty(M, dtype=torch.float32, device="cuda")
+            pct.pct_get_image(ctx, img, M)
+            out["image_finite"] = bool(torch.isfinite(img).all().item())
+            out["image_mean_central"] = float(img.view(cfg.nz, cfg.ny, cfg.nx)[cfg.nz // 2, cfg.ny // 2 - 8:cfg.ny // 2 + 8,
+                                                                           cfg.nx // 2 - 8:cfg.nx // 2 + 8].mean().item())
+        finally:
+            pct.pct_destroy(ctx)
+
+        # ---- end to end through the C ABI from pinned host memory ----
+        if not args.no_e2e:
+            host = {}
+            for k, v in P.items():
+                h = torch.empty(v.shape, dtype=v.dtype, pin_memory=True)
+                h.copy_(v)
+                host[k] = h
+            torch.cuda.synchronize()
+            h2d = sum(host[k].numel() * host[k].element_size() for k in host)
+            img_host = torch.empty(M, dtype=torch.float32, pin_memory=True)
+            ctx = pct.pct_create(cfg.nx, cfg.ny, cfg.nz, cfg.h, cfg.u_in, cfg.u_out, stream.cuda_stream)
+            try:
+                def e2e_step():
+                    pct.pct_set_histories_host(ctx, n, host)
+                    pct.pct_iterate(ctx, lam, B, 1)
+                    pct.pct_get_image(ctx, img_host, M)  # synchronises
+
+                e2e_step()  # warm-up (allocations, graph instantiation)
+                barrier()
+                torch.cuda.synchronize()
+                e0.record()
+                for _ in range(args.e2e_steps):
+                    e2e_step()
+                e1.record()
+                torch.cuda.synchronize()
+                barrier()
+                ms = max_over_ranks(e0.elapsed_time(e1))
+                out["e2e"] = {"value": world * n * args.e2e_steps / (ms * 1e-3), "unit": UNIT, "h2d_bytes_per_step": h2d,
+                              "d2h_bytes_per_step": 4 * M, "steps": args.e2e_steps, "ms_per_step": ms / args.e2e_steps,
+                              "path": "pct_set_histories_host (pinned host SoA) -> pct_iterate(1 sweep) -> pct_get_image (pinned host)"}
+            finally:
+                pct.pct_destroy(ctx)
+            del host
+
+    # ---- CPU baseline: the oracle on this box's host cores, rank 0, N = 1 only ----
+    cpu = None
+    if rank == 0 and world == 1 and not args.no_cpu:
+        n_s = min(n, 64 * B)
+        Hs = {k: v[:n_s].cpu().numpy() for k, v in D.items() if k not in ("proj_cos", "proj_sin")}
+        Hs["proj"] = Hs["proj"].view(np.uint16)
+        Hs["proj_cos"], Hs["proj_sin"] = D["proj_cos"].cpu().numpy(), D["proj_sin"].cpu().numpy()
+        rate, cores, nb, dt = cpu_oracle_rate(cfg, Hs, args.cpu_seconds)
+        cpu = {"value": rate, "unit": UNIT, "cores": cores, "kind": "oracle", "seconds": dt,
+               "sample": "first %d DROP blocks (%d histories) of the same workload, one sweep from x0 = 0" % (nb, nb * B)}
+
+    if world > 1:
+        dist.destroy_process_group()
+    if rank != 0:
+        return
+
+    peaks = measured_peaks()
+    st, prof = out["stats"], out["prof"]
+    seg_per_hist = st["segments"] / max(1, st["histories"])
+    nnz_per_hist = st["nnz"] / max(1, st["histories"])
+    k_ms = prof["accumulate_ms"] / prof["blocks"]  # average device time of one launch
+    hist_per_launch = n / prof["blocks"]
+    ops = OPS_PER_SEGMENT * seg_per_hist * hist_per_launch
+    alu_peak = SM_COUNT * LANES_PER_SM * peaks["sm_max_mhz"] * 1e6 / 1e12  # T thread-instructions/s
+    alu_ach = ops / (k_ms * 1e-3) / 1e12
+    hbm_ach = HBM_BYTES_PER_HISTORY * hist_per_launch / (k_ms * 1e-3) / 1e9
+    l2_bytes = (4.0 * seg_per_hist + 8.0 * nnz_per_hist) * hist_per_launch
+    roofline = {
+        "kernel": "pct::k_drop_block (fused hull+MLP+walk+projection+scatter)", "bound": "alu",
+        "achieved": alu_ach, "peak": alu_peak, "unit": "Tinst/s", "frac": alu_ach / alu_peak,
+        "peak_source": "148 SM x 128 fp32 lanes x %.0f MHz (MEASURED_PEAKS.json sm_max_mhz, %s)" % (peaks["sm_max_mhz"], peaks["source"]),
+        "algorithmic": "%d fp32/int ops per path segment (DESIGN.md Roofline) x %.1f segments/history x %d histories/launch" % (
+            OPS_PER_SEGMENT, seg_per_hist, hist_per_launch),
+        "kernel_ms": k_ms, "launches_timed": prof["blocks"],
+        "kernel_share_of_step": prof["accumulate_ms"] / prof["sweep_ms"],
+        "update_kernel_ms": prof["update_ms"] / prof["blocks"],
+        "timing": "CUDA events around every launch on the kernels' stream (pct_profile_sweep), one sweep of the timed workload",
+        "traffic": None,
+        "hbm": {"achieved": hbm_ach, "peak": peaks["hbm_gbs"], "unit": "GB/s", "frac": hbm_ach / peaks["hbm_gbs"],
+                "peak_source": peaks["source"], "algorithmic": "38 B/history"},
+        "l2_useful": {"achieved": l2_bytes / (k_ms * 1e-3) / 1e9, "unit": "GB/s",
+                      "algorithmic": "4 B gather/segment + 8 B (Delta,c) reduction/non-zero"},
+    }
+    line = {
+        "metric": METRIC, "value": out["value"], "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
+        "ms_per_step": out["ms_per_step"], "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+        "dtype": "f32", "data": "synthetic",
+        "config": {"workload": cfg.workload, "histories": n, "grid": [cfg.nx, cfg.ny, cfg.nz], "voxel_mm": cfg.h,
+                   "angles": cfg.n_angles, "block_size": B, "blocks_per_step": n_blocks, "lambda": lam,
+                   "step": "one DROP sweep (iteration) over all histories",
+                   "l2": "inputs larger than L2 (histories %.1f GB, image+accumulator %.0f MB vs 126 MB L2)" % (
+                       38.0 * n / 1e9, 12.0 * M / 1e6),
+                   "multi_gpu": "replicas only", "histories_override": args.histories is not None},
+        "clocks": out["clocks"], "gpu_launches": 2 * n_blocks * args.steps,
+        "segments_per_history": seg_per_hist, "nonzeros_per_history": nnz_per_hist,
+        "skipped_fraction": 1.0 - st["rows"] / max(1, st["histories"]),
+        "image_finite": out["image_finite"], "image_mean_central": out["image_mean_central"],
+        "roofline": roofline,
+    }
+    if "e2e" in out:
+        line["e2e"] = out["e2e"]
+    if cpu is not None:
+        line["cpu_baseline"] = cpu
+    print(json.dumps(line))
+
+
+def main():
+    args = parse_args()
+    if args.impl == "reference":
+        run_reference(args)
+    else:
+        run_ours(args)
+
+
+if __name__ == "__main__":
+    main()

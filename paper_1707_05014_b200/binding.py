@@ -57,13 +57,14 @@ def lib():
         L.pct_version.restype = C.c_char_p
         L.pct_debug_rows.argtypes = [vp, i64, i64, C.c_int32, vp, vp, vp, vp, vp, vp]
         L.pct_debug_block.argtypes = [vp, i64, i64, vp, vp]
+        L.pct_profile_sweep.argtypes = [vp, C.c_float, i64, C.POINTER(C.c_float)]
         _lib = L
     return _lib
 
 
 EXPORTS = ("pct_create", "pct_set_histories", "pct_set_histories_host", "pct_iterate", "pct_get_image",
            "pct_set_image", "pct_synchronize", "pct_get_stats", "pct_destroy", "pct_last_error", "pct_version",
-           "pct_debug_rows", "pct_debug_block")
+           "pct_debug_rows", "pct_debug_block", "pct_profile_sweep")
 
 
 def _ptr(a):
@@ -150,3 +151,10 @@ def pct_debug_rows(ctx, first, count, max_seg, nseg, nnz, seg_idx=None, seg_len=
 
 def pct_debug_block(ctx, first, count, delta, cnt):
     _check(ctx, lib().pct_debug_block(ctx, int(first), int(count), _ptr(delta), _ptr(cnt)))
+
+
+def pct_profile_sweep(ctx, lam, block_size):
+    """One sweep with CUDA events around every launch -> dict of device times (include/pct.h)."""
+    out = (C.c_float * 4)()
+    _check(ctx, lib().pct_profile_sweep(ctx, float(lam), int(block_size), out))
+    return dict(accumulate_ms=out[0], update_ms=out[1], sweep_ms=out[2], blocks=int(out[3]))

@@ -376,3 +376,52 @@ extern "C" int pct_debug_block(pct_ctx* c, int64_t first, int64_t count, float* 
     CUDA_TRY(c, cudaMemsetAsync(c->ctrl, 0, sizeof(Ctrl), c->stream));
     return PCT_OK;
 }
+
+extern "C" int pct_profile_sweep(pct_ctx* c, float lambda, int64_t block_size, float out_ms[4]) {
+    if (!c) return PCT_EINVAL;
+    if (!out_ms) return fail(c, PCT_EINVAL, "pct_profile_sweep: out_ms is NULL");
+    if (!c->have_hist) return fail(c, PCT_ESTATE, "pct_profile_sweep: no histories set");
+    if (!(lambda > 0.0f) || !(lambda < 2.0f)) return fail(c, PCT_EINVAL, "pct_profile_sweep: lambda must be in (0, 2)");
+    if (block_size < 1 || block_size > (1LL << 24)) return fail(c, PCT_EINVAL, "pct_profile_sweep: block_size must be in [1, 2^24]");
+    const long long n_blocks = (c->n + block_size - 1) / block_size;
+    const int kChunk = 256;  // blocks per batch of events
+    cudaEvent_t ev[2 * kChunk + 1];
+    int made = 0;
+    int rc = PCT_OK;
+    double drop_ms = 0.0, upd_ms = 0.0, total_ms = 0.0;
+    auto body = [&]() -> int {
+        for (; made < 2 * kChunk + 1; ++made) CUDA_TRY(c, cudaEventCreate(&ev[made]));
+        CUDA_TRY(c, cudaMemsetAsync(c->ctrl, 0, sizeof(Ctrl), c->stream));
+        const DropArgs a = drop_args(c, block_size, -1, 0);
+        for (long long b0 = 0; b0 < n_blocks; b0 += kChunk) {
+            const int nb = (int)(n_blocks - b0 < kChunk ? n_blocks - b0 : kChunk);
+            CUDA_TRY(c, cudaEventRecord(ev[0], c->stream));
+            for (int i = 0; i < nb; ++i) {
+                CUDA_TRY(c, launch_drop_block(a, c->drop_grid, c->stream));
+                CUDA_TRY(c, cudaEventRecord(ev[2 * i + 1], c->stream));
+                CUDA_TRY(c, launch_update(c->x, c->acc, c->n_voxels, lambda, c->ctrl, n_blocks, c->stream));
+                CUDA_TRY(c, cudaEventRecord(ev[2 * i + 2], c->stream));
+            }
+            CUDA_TRY(c, cudaStreamSynchronize(c->stream));
+            for (int i = 0; i < nb; ++i) {
+                float d = 0.f, u = 0.f;
+                CUDA_TRY(c, cudaEventElapsedTime(&d, ev[2 * i], ev[2 * i + 1]));
+                CUDA_TRY(c, cudaEventElapsedTime(&u, ev[2 * i + 1], ev[2 * i + 2]));
+                drop_ms += d;
+                upd_ms += u;
+            }
+            float t = 0.f;
+            CUDA_TRY(c, cudaEventElapsedTime(&t, ev[0], ev[2 * nb]));
+            total_ms += t;
+        }
+        return PCT_OK;
+    };
+    rc = body();
+    for (int i = 0; i < made; ++i) cudaEventDestroy(ev[i]);
+    if (rc != PCT_OK) return rc;
+    out_ms[0] = (float)drop_ms;
+    out_ms[1] = (float)upd_ms;
+    out_ms[2] = (float)total_ms;
+    out_ms[3] = (float)n_blocks;
+    return PCT_OK;
+}

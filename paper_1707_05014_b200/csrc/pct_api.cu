@@ -125,6 +125,7 @@ extern "C" int pct_create(pct_ctx** out, int nx, int ny, int nz, float h, float 
     g.zmax = (0.5f * (float)nz) * h;
     g.u_in = u_in; g.u_out = u_out;
     g.hx = 0.5f * (float)nx; g.hy = 0.5f * (float)ny; g.hz = 0.5f * (float)nz;
+    g.fnx = (float)nx; g.fny = (float)ny; g.fnz = (float)nz;
     if (!(u_in <= -R) || !(u_out >= R) || !isfinite(u_in) || !isfinite(u_out))
         return fail(nullptr, PCT_EINVAL, "pct_create: tracker planes must lie outside the hull (u_in <= -R_h, u_out >= R_h)");
     pct_ctx* c = new (std::nothrow) pct_ctx;

@@ -4,20 +4,32 @@
 //                 -> scatter of (r_i a_ij, 1) into the block accumulator (R12).
 //                 One WARP walks one history; lane l owns the CONTIGUOUS chunk of segments
 //                 [l*C, (l+1)*C), C = ceil((K+1)/32) (the MLP node at depth k*h is closed-form in
-//                 k, there is no recurrence along the path).  A lane keeps its <= CMAX (voxel,
-//                 length, x) triples in registers between the dot-product pass and the scatter
-//                 pass, so the path is computed once per sweep and never touches memory; runs of
-//                 equal voxels are merged sequentially inside a lane, and the at most 31 lane
-//                 seams are patched with three shuffles.
+//                 k, there is no recurrence along the path) and walks it in a rolled loop, merging
+//                 runs of equal voxels and summing ||a_i||^2 as it goes; the at most 31 lane seams
+//                 are patched with three shuffles.  The row (voxel, length, run-head flag) goes to a
+//                 per-warp buffer in SHARED memory and is read back segment-major (lane l takes
+//                 segments 32 i + l) by the gather pass (a_i.x) and the scatter pass, so that
+//                 neighbouring lanes touch neighbouring voxels and their L2 requests coalesce.  The
+//                 path is computed once per sweep and never touches global memory.
 //   k_update      x_j += lambda * Delta_j / max(1, c_j); accumulator zeroed; DROP block index advanced.
 //   k_rows        inspection: the same walk, rows written out instead of consumed.
 #include "pct_internal.h"
 
 namespace pct {
 
-constexpr int kWarpsPerCta = 8;
+#ifndef PCT_WARPS_PER_CTA
+#define PCT_WARPS_PER_CTA 8
+#endif
+#ifndef PCT_CTAS_PER_SM
+#define PCT_CTAS_PER_SM 3  // register budget of k_drop_block: 65536 / (3 * 256) -> 80 per thread
+#endif
+#ifndef PCT_BATCH
+#define PCT_BATCH 16
+#endif
+constexpr int kWarpsPerCta = PCT_WARPS_PER_CTA;
 constexpr int kThreads = kWarpsPerCta * 32;
-constexpr int kBatch = 8;  // histories a warp takes from the work queue per trip (at most)
+constexpr int kCtasPerSm = PCT_CTAS_PER_SM;
+constexpr int kBatch = PCT_BATCH;  // histories a warp takes from the work queue per trip (at most)
 
 // Sigma1^-1 table in shared memory: entry k sits at slot k + (k >> 3), so that the 8 lanes of a
 // quarter warp, which read entries C apart, fall into different 16-byte bank groups for every
@@ -26,9 +38,23 @@ constexpr int kBatch = 8;  // histories a warp takes from the work queue per tri
 __host__ __device__ inline int tab_slot(int k) { return k + (k >> 3); }
 __host__ __device__ inline int tab_slots(int nmin) { return (tab_slot(nmin + 33) + 4) & ~3; }
 
-size_t drop_smem_bytes(int nmin) {
-    return sizeof(float4) * tab_slots(nmin) + (size_t)kWarpsPerCta * kBatch * sizeof(PathState);
+__host__ __device__ inline int row_slot(int s);
+__host__ __device__ inline int row_slots(int cmax);
+
+// Dynamic shared memory of a CTA: Sigma1^-1 table | PathState[warps][kBatch] | row buffer[warps].
+struct SmemLayout {
+    int state_off, row_off, row_slots, total;
+};
+__host__ __device__ inline SmemLayout smem_layout(int nmin) {
+    SmemLayout l;
+    l.state_off = (int)sizeof(float4) * tab_slots(nmin);
+    l.row_off = l.state_off + kWarpsPerCta * kBatch * (int)sizeof(PathState);
+    l.row_slots = row_slots((nmin + 32) >> 5);  // K <= nmin: at most ceil((nmin + 1) / 32) segments per lane
+    l.total = l.row_off + kWarpsPerCta * l.row_slots * (int)sizeof(float2);
+    return l;
 }
+
+size_t drop_smem_bytes(int nmin) { return (size_t)smem_layout(nmin).total; }
 
 __device__ __forceinline__ float warp_sum(float v) {
 #pragma unroll
@@ -68,140 +94,112 @@ struct EmitPtrs {
     float *seg_len, *row_len, *nodes;
 };
 
-// One lane's part of the row of one history, in registers.
-template <int CMAX>
-struct LaneRow {
-    int lin[CMAX];    // voxel of segment k0 + c, -1: outside the grid or past the end of the path
-    float len[CMAX];  // its length, 0 where lin < 0
-    unsigned heads;   // bit c: segment k0 + c starts a run of equal voxels (R10) = one non-zero of the row
-    int C;            // segments per lane of this history
-};
+// ---- row buffer of one warp (shared memory) --------------------------------------------------
+// Entry s belongs to segment s of the history being walked: (voxel, length).  voxel = -1: outside
+// the grid or past the end of the path (length 0).  The SIGN BIT of the length is the run-head
+// flag: set iff the segment starts a run of equal voxels (R10), i.e. iff it counts as one non-zero
+// of the row.  The walk writes the buffer lane-chunked (lane l owns segments l*C .. l*C+C-1); the
+// gather and scatter passes read it segment-major (lane l takes segments 32 i + l), so that
+// neighbouring lanes touch neighbouring voxels and their L2 requests coalesce.  Physical slot
+// s + (s >> 5): reads are conflict-free, writes at most 2-way for every chunk size.
+__host__ __device__ inline int row_slot(int s) { return s + (s >> 5); }
+__host__ __device__ inline int row_slots(int cmax) { return row_slot(32 * cmax) + 2; }
 
-__device__ __forceinline__ void emit_segment(const EmitPtrs& em, int k, int K, int lin, float len, const float3 a,
-                                             const float3 exitP) {
-    if (em.seg_idx) em.seg_idx[k] = lin;
-    if (em.seg_len) em.seg_len[k] = len;
+__device__ __forceinline__ void emit_node(const EmitPtrs& em, int k, const float3 a) {
     if (em.nodes) {
         em.nodes[3 * k + 0] = a.x;
         em.nodes[3 * k + 1] = a.y;
         em.nodes[3 * k + 2] = a.z;
-        if (k == K) {
-            em.nodes[3 * k + 3] = exitP.x;
-            em.nodes[3 * k + 4] = exitP.y;
-            em.nodes[3 * k + 5] = exitP.z;
-        }
     }
 }
 
-// Walk of one history by one warp (steps 3-4 of the rule).  Fills the lane's part of the row,
-// returns the lane's parts of a_i.x (GATHER), ||a_i||^2 and the non-zero count.
+// Sequential merge of consecutive equal voxels inside one lane (R10) and the lane's part of ||a_i||^2.
+struct MergeState {
+    int run_idx;      // voxel of the current run (-2: none yet)
+    float run_len;    // its length so far (this lane's part)
+    float first_len;  // length of the lane's first run (this lane's part), set when the second run starts
+    int n_fresh;      // runs started so far (a dropped segment, voxel -1, starts a run here too)
+    int nnz;          // run heads with a voxel inside the grid
+    float nrm;        // sum of squares of the FINISHED runs
+};
+
+// Segment `seg` of the lane, from node a to node b: voxel + length (rule step 4), merge, row-buffer entry.
+template <bool EMIT>
+__device__ __forceinline__ void take_segment(const Geom& g, const float3 a, const float3 b, int seg, int K, MergeState& m,
+                                             float2* row, const EmitPtrs& em) {
+    int lin;
+    float len;
+    segment(g, a, b, lin, len);
+    const bool ok = (seg <= K) && lin >= 0;
+    if (EMIT) {  // a dropped segment has no entry in the row; the inspection kernel still reports its length
+        if (seg <= K && !ok && em.seg_len) em.seg_len[seg] = len;
+    }
+    lin = ok ? lin : -1;
+    len = ok ? len : 0.0f;
+    const bool fresh = lin != m.run_idx;
+    if (fresh) {
+        m.nrm = __fmaf_rn(m.run_len, m.run_len, m.nrm);  // the finished run
+        if (m.n_fresh == 1) m.first_len = m.run_len;
+        ++m.n_fresh;
+    }
+    m.run_len = fresh ? len : m.run_len + len;
+    m.run_idx = lin;
+    const bool head = fresh && lin >= 0;
+    m.nnz += head ? 1 : 0;
+    row[row_slot(seg)] = make_float2(__int_as_float(lin), head ? -len : len);
+    if (EMIT) {
+        if (seg <= K) emit_node(em, seg, a);
+    }
+}
+
+// Walk of one history by one warp (steps 3-4 of the rule): fills the warp's row buffer, returns the
+// lane's part of ||a_i||^2 and of the non-zero count.
 //
-// Lane l evaluates the MLP at nodes k0+1 .. k0+C (k0 = l*C); its segment c joins nodes k0+c and
-// k0+c+1, so segments 1..C-1 need only the lane's own nodes and segment 0 starts at the LAST node
-// of lane l-1, fetched with one shuffle after the node loop (lane 0: the hull entry point).
-// Lanes past the end of the path run the same instructions on harmless values and are masked.
-template <int CMAX, bool GATHER, bool EMIT>
-__device__ __forceinline__ void walk_history(const Geom& g, const PathState& S, const float4* s_tab,
-                                             const float* __restrict__ x, int lane, LaneRow<CMAX>& row, float& dot,
+// Lane l owns segments k0 .. k0+C-1 (k0 = l*C), i.e. it needs nodes k0 .. k0+C.  It evaluates its
+// LAST node (k0+C) first and hands it to lane l+1 as that lane's start node with one shuffle (lane
+// 0 starts at the hull entry point), then walks nodes k0+1 .. k0+C-1 in a rolled loop -- the MLP
+// node at depth k*h is closed-form in k, there is no recurrence along the path.  Lanes past the end
+// of the path run the same instructions on harmless values and are masked.
+template <bool EMIT>
+__device__ __forceinline__ void walk_history(const Geom& g, const PathState& S, const float4* s_tab, int lane, float2* row,
                                              float& nrm, int& nnz, const EmitPtrs& em) {
     const PathState st = S;  // shared memory -> registers, once per history
     const int K = st.K;
     const int C = (K + 32) >> 5;  // ceil((K + 1) / 32) segments per lane
     const int k0 = lane * C;
-    row.C = C;
     const float3 exitP = to_object(st, st.t2, st.u2, st.v2);  // node K+1: the hull exit point, assigned (R9)
-    float xv[CMAX];
-    float3 n1 = exitP, prv = exitP;
-#pragma unroll
-    for (int j = 1; j <= CMAX; ++j) {
-        if (j < CMAX) {
-            row.lin[j] = -1;
-            row.len[j] = 0.0f;
-            xv[j] = 0.0f;
-        }
-        if (j <= C) {  // warp-uniform
-            const int k = k0 + j;  // node index
-            float3 nd = mlp_node(g, st, s_tab[tab_slot(k)], k);
-            if (k > K) nd = exitP;
-            if (j == 1) {
-                n1 = nd;
-            } else {  // segment k-1 = slot j-1, between the lane's nodes j-1 and j
-                int lin;
-                float len;
-                segment(g, prv, nd, lin, len);
-                const bool ok = (k - 1 <= K) && lin >= 0;
-                row.lin[j - 1] = ok ? lin : -1;
-                row.len[j - 1] = ok ? len : 0.0f;
-                if (GATHER) {
-                    if (ok) xv[j - 1] = __ldg(x + lin);
-                }
-                if (EMIT) {
-                    if (k - 1 <= K) emit_segment(em, k - 1, K, lin, len, prv, exitP);
-                }
-            }
-            prv = nd;
-        }
+    float3 last = mlp_node(g, st, s_tab[tab_slot(k0 + C)], k0 + C);
+    if (k0 + C > K) last = exitP;
+    float3 prv;
+    prv.x = __shfl_up_sync(0xffffffffu, last.x, 1);
+    prv.y = __shfl_up_sync(0xffffffffu, last.y, 1);
+    prv.z = __shfl_up_sync(0xffffffffu, last.z, 1);
+    if (lane == 0) prv = to_object(st, st.t0, st.u0, st.v0);  // node 0: the hull entry point (R9)
+    MergeState m{-2, 0.0f, 0.0f, 0, 0, 0.0f};
+#pragma unroll 1
+    for (int c = 1; c < C; ++c) {
+        const int k = k0 + c;  // node index; segment k-1 ends here
+        float3 nd = mlp_node(g, st, s_tab[tab_slot(k)], k);
+        if (k > K) nd = exitP;
+        take_segment<EMIT>(g, prv, nd, k - 1, K, m, row, em);
+        prv = nd;
     }
-    {  // slot 0: from the last node of the previous lane (= node k0) to the lane's first node
-        float3 start;
-        start.x = __shfl_up_sync(0xffffffffu, prv.x, 1);
-        start.y = __shfl_up_sync(0xffffffffu, prv.y, 1);
-        start.z = __shfl_up_sync(0xffffffffu, prv.z, 1);
-        if (lane == 0) start = to_object(st, st.t0, st.u0, st.v0);  // node 0: the hull entry point (R9)
-        int lin;
-        float len;
-        segment(g, start, n1, lin, len);
-        const bool ok = (k0 <= K) && lin >= 0;
-        row.lin[0] = ok ? lin : -1;
-        row.len[0] = ok ? len : 0.0f;
-        xv[0] = 0.0f;
-        if (GATHER) {
-            if (ok) xv[0] = __ldg(x + lin);
-        }
-        if (EMIT) {
-            if (k0 <= K) emit_segment(em, k0, K, lin, len, start, exitP);
-        }
+    take_segment<EMIT>(g, prv, last, k0 + C - 1, K, m, row, em);
+    if (EMIT) {
+        if (k0 <= K && K < k0 + C) emit_node(em, K + 1, exitP);
     }
-    // ---- a_i.x, and the merge of consecutive equal voxels (R10), sequential inside the lane ----
-    dot = 0.0f;
-    nrm = 0.0f;
-    nnz = 0;
-    unsigned heads = 0u;
-    int run_idx = -2;        // voxel of the current run (-2: none yet)
-    float run_len = 0.0f;    // its length so far (this lane's part)
-    float first_len = 0.0f;  // length of the lane's first run (this lane's part)
-    bool whole = true;       // the lane's whole chunk is one run
-#pragma unroll
-    for (int c = 0; c < CMAX; ++c) {
-        if (c < C) {
-            dot = __fmaf_rn(row.len[c], xv[c], dot);
-            const bool fresh = row.lin[c] != run_idx;
-            if (fresh) {
-                nrm = __fmaf_rn(run_len, run_len, nrm);  // the finished run
-                if (c > 0 && whole) {
-                    first_len = run_len;
-                    whole = false;
-                }
-                run_idx = row.lin[c];
-                run_len = row.len[c];
-                if (run_idx >= 0) {
-                    heads |= 1u << c;
-                    ++nnz;
-                }
-            } else {
-                run_len += row.len[c];
-            }
-        }
-    }
-    nrm = __fmaf_rn(run_len, run_len, nrm);
-    if (whole) first_len = run_len;
+    m.nrm = __fmaf_rn(m.run_len, m.run_len, m.nrm);
+    const bool whole = m.n_fresh == 1;  // the lane's whole chunk is one run
+    if (whole) m.first_len = m.run_len;
     // ---- lane seams: the lane's first run may continue the previous lane's last run ----------
     // With p = this lane's part and q = the part in earlier lanes, (q + p)^2 = q^2 + 2qp + p^2:
     // q^2 is already in the earlier lanes' sums, p^2 in this lane's, the seam adds 2qp.
-    const int prev_idx = __shfl_up_sync(0xffffffffu, run_idx, 1);
-    const float prev_len = __shfl_up_sync(0xffffffffu, run_len, 1);
+    const float2 e0 = row[row_slot(k0)];
+    const int lin0 = __float_as_int(e0.x);
+    const int prev_idx = __shfl_up_sync(0xffffffffu, m.run_idx, 1);
+    const float prev_len = __shfl_up_sync(0xffffffffu, m.run_len, 1);
     const bool prev_whole = __shfl_up_sync(0xffffffffu, (int)whole, 1) != 0;
-    const bool cont = lane > 0 && row.lin[0] >= 0 && row.lin[0] == prev_idx;
+    const bool cont = lane > 0 && lin0 >= 0 && lin0 == prev_idx;
     const float base = cont ? prev_len : 0.0f;
     float carry = base;  // length of the lane's first run that lies in earlier lanes
     if (__any_sync(0xffffffffu, cont && prev_whole)) {
@@ -215,27 +213,112 @@ __device__ __forceinline__ void walk_history(const Geom& g, const PathState& S, 
         }
     }
     if (cont) {
-        heads &= ~1u;
-        --nnz;
-        nrm = __fmaf_rn(2.0f * carry, first_len, nrm);
+        row[row_slot(k0)] = make_float2(e0.x, fabsf(e0.y));  // not a run head after all
+        --m.nnz;
+        m.nrm = __fmaf_rn(2.0f * carry, m.first_len, m.nrm);
     }
-    row.heads = heads;
-    if (EMIT) {
-        if (em.row_len) {
+    nrm = m.nrm;
+    nnz = m.nnz;
+    __syncwarp();  // the row buffer is complete: the passes below read it segment-major
+}
+
+// ---- segment-major passes over the row buffer ------------------------------------------------
+// Lane l reads segments 32 i + l: physical slot row_slot(32 i + l) = 33 i + l.  The passes are
+// instantiated for an exact number N of segments per lane (no per-slot bounds test) and
+// dispatched on the warp-uniform C.
+
+// (Delta_j, c_j) += (v, cnt): one 64-bit vector reduction, no return value, predicated on lin >= 0.
+__device__ __forceinline__ void red_add_v2(float2* acc, int lin, float v, float cnt) {
+    asm volatile(
+        "{\n\t.reg .pred p;\n\t.reg .u64 ad;\n\t"
+        "setp.ge.s32 p, %1, 0;\n\t"
+        "mad.wide.s32 ad, %1, 8, %0;\n\t"
+        "@p red.global.add.v2.f32 [ad], {%2, %3};\n\t}"
+        :: "l"(acc), "r"(lin), "f"(v), "f"(cnt) : "memory");
+}
+
+template <int N>
+__device__ __forceinline__ float gather_n(const float2* rl, const float* __restrict__ x) {
+    float2 e[N];
+    float xv[N];
 #pragma unroll
-            for (int c = 0; c < CMAX; ++c)
-                if (c < C && k0 + c <= K) em.row_len[k0 + c] = ((heads >> c) & 1u) ? 1.0f : 0.0f;
-        }
+    for (int u = 0; u < N; ++u) e[u] = rl[33 * u];
+#pragma unroll
+    for (int u = 0; u < N; ++u) {
+        const int lin = __float_as_int(e[u].x);
+        xv[u] = 0.0f;
+        if (lin >= 0) xv[u] = __ldg(x + lin);
+    }
+    float dot = 0.0f;
+#pragma unroll
+    for (int u = 0; u < N; ++u) dot = __fmaf_rn(fabsf(e[u].y), xv[u], dot);
+    return dot;
+}
+
+template <int N>
+__device__ __forceinline__ void scatter_n(const float2* rl, float2* acc, float r) {
+#pragma unroll
+    for (int u = 0; u < N; ++u) {
+        const float2 e = rl[33 * u];
+        red_add_v2(acc, __float_as_int(e.x), r * fabsf(e.y), __float_as_int(e.y) < 0 ? 1.0f : 0.0f);
     }
 }
 
-// Work queue of one DROP block: items of kBatch histories first, then (the last ~1/8 of the
-// block) items of kBatch/4, so that the warps run dry within a couple of histories of each
-// other.  Small blocks get smaller items so that they still spread over the whole grid.
+#define PCT_SWITCH_N(n, CALL)        \
+    switch (n) {                     \
+        case 1: CALL(1); break;      \
+        case 2: CALL(2); break;      \
+        case 3: CALL(3); break;      \
+        case 4: CALL(4); break;      \
+        case 5: CALL(5); break;      \
+        case 6: CALL(6); break;      \
+        case 7: CALL(7); break;      \
+        default: break;              \
+    }
+
+// a_i.x (a4): gather of x through L2, C segments per lane.
+__device__ __forceinline__ float gather_row(const float2* row, int lane, int C, const float* __restrict__ x) {
+    const float2* rl = row + lane;
+    float dot = 0.0f;
+    int i = 0;
+    for (; i + 8 <= C; i += 8) dot += gather_n<8>(rl + 33 * i, x);
+#define PCT_G(N) dot += gather_n<N>(rl + 33 * i, x)
+    PCT_SWITCH_N(C - i, PCT_G);
+#undef PCT_G
+    return dot;
+}
+
+// scatter (a5): (Delta_j, c_j) += (r a_ij, 1 per run head).
+__device__ __forceinline__ void scatter_row(const float2* row, int lane, int C, float2* acc, float r) {
+    const float2* rl = row + lane;
+    int i = 0;
+    for (; i + 8 <= C; i += 8) scatter_n<8>(rl + 33 * i, acc, r);
+#define PCT_S(N) scatter_n<N>(rl + 33 * i, acc, r)
+    PCT_SWITCH_N(C - i, PCT_S);
+#undef PCT_S
+}
+
+// Work queue of one DROP block.  Phase 0 is STATIC: warp w of the grid owns item w (about half of
+// its fair share of the block, at most kBatch histories) without touching the ticket counter, so
+// the launch does not open with every warp hitting one address.  The rest is guided
+// self-scheduling over one atomic ticket counter: items of half, a quarter, ... of the static size,
+// each phase covering half of what is left, down to single histories -- a warp that draws one of
+// the last big items stays busy for that many walks, so the work behind it must be fine-grained
+// enough for the other warps to fill that time.  Small blocks get smaller items so that they still
+// spread over the whole grid.
+#ifndef PCT_QUEUE_HEAD_SHIFT
+#define PCT_QUEUE_HEAD_SHIFT 2  // dynamic phase 1 covers left - (left >> shift) histories
+#endif
+#ifndef PCT_QUEUE_DIV
+#define PCT_QUEUE_DIV 2  // static items: 1/DIV of a warp's fair share of the block
+#endif
+constexpr int kPhases = 4;
 struct Queue {
     long long first, count;
-    int big, small;            // histories per item in the two phases
-    unsigned long long n_big;  // items of the first phase
+    int size[kPhases];                  // histories per item
+    unsigned long long item0[kPhases];  // first ticket of the phase
+    long long hist0[kPhases];           // first history of the phase (relative to `first`)
+    unsigned long long n_static;        // tickets [0, n_static) are owned by warps, not drawn
     unsigned long long n_items;
 };
 
@@ -243,52 +326,77 @@ __device__ __forceinline__ Queue make_queue(long long first, long long count, lo
     Queue q;
     q.first = first;
     q.count = count;
-    long long big = count / (4 * n_warps);
+    long long big = count / (PCT_QUEUE_DIV * n_warps);
     big = big < 1 ? 1 : (big > kBatch ? kBatch : big);
-    const long long small = big >= 4 ? big / 4 : 1;
-    const long long nb = (count - count / 8) / big;
-    const long long rest = count - nb * big;
-    q.big = (int)big;
-    q.small = (int)small;
-    q.n_big = (unsigned long long)nb;
-    q.n_items = (unsigned long long)(nb + (rest + small - 1) / small);
+    long long done = 0;
+    unsigned long long items = 0;
+#pragma unroll
+    for (int p = 0; p < kPhases; ++p) {
+        long long sz = big >> p;
+        sz = sz < 1 ? 1 : sz;
+        const long long left = count - done;
+        long long n;
+        if (p == 0) {
+            n = left / sz < n_warps ? left / sz : n_warps;  // one static item per warp
+        } else if (p == kPhases - 1) {
+            n = (left + sz - 1) / sz;  // the last phase takes the ragged end
+        } else {
+            n = (left - (left >> (p == 1 ? PCT_QUEUE_HEAD_SHIFT : 1))) / sz;
+        }
+        q.size[p] = (int)sz;
+        q.item0[p] = items;
+        q.hist0[p] = done;
+        items += (unsigned long long)n;
+        done += n * sz;
+        if (done > count) done = count;
+        if (p == 0) q.n_static = (unsigned long long)n;
+    }
+    q.n_items = items;
     return q;
 }
 
-template <int CMAX>
-__global__ void __launch_bounds__(kThreads, 2) k_drop_block(const DropArgs a) {
+__device__ __forceinline__ void queue_item(const Queue& q, unsigned long long w, long long& i0, int& cnt) {
+    int p = 0;
+#pragma unroll
+    for (int t = 1; t < kPhases; ++t) p = w >= q.item0[t] ? t : p;
+    const long long rel = q.hist0[p] + (long long)(w - q.item0[p]) * q.size[p];
+    i0 = q.first + rel;
+    const long long left = q.count - rel;
+    cnt = left < q.size[p] ? (int)left : q.size[p];
+}
+
+__global__ void __launch_bounds__(kThreads, kCtasPerSm) k_drop_block(const DropArgs a) {
     extern __shared__ __align__(16) unsigned char smem_raw[];
     const Geom g = a.g;
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    const SmemLayout lay = smem_layout(g.nmin);
     float4* s_tab = reinterpret_cast<float4*>(smem_raw);
-    PathState* s_state = reinterpret_cast<PathState*>(smem_raw + sizeof(float4) * tab_slots(g.nmin)) + warp * kBatch;
-    stage_table(s_tab, a.tab, g.nmin);
-
-    long long first = a.first, count = a.count;
-    if (first < 0) {
-        first = a.ctrl->block * a.block_size;
-        count = a.n - first < a.block_size ? a.n - first : a.block_size;
+    PathState* s_state = reinterpret_cast<PathState*>(smem_raw + lay.state_off) + warp * kBatch;
+    float2* row = reinterpret_cast<float2*>(smem_raw + lay.row_off) + warp * lay.row_slots;
+    __shared__ Queue q;  // one copy per CTA: the phase of a ticket is looked up by index
+    if (threadIdx.x == 0) {
+        long long first = a.first, count = a.count;
+        if (first < 0) {
+            first = a.ctrl->block * a.block_size;
+            count = a.n - first < a.block_size ? a.n - first : a.block_size;
+        }
+        q = make_queue(first, count, (long long)gridDim.x * kWarpsPerCta);
     }
-    const Queue q = make_queue(first, count, (long long)gridDim.x * kWarpsPerCta);
+    stage_table(s_tab, a.tab, g.nmin);  // (ends with __syncthreads: q is visible)
     unsigned long long rows = 0, nnz_total = 0, segs = 0;
     const EmitPtrs no_emit{nullptr, nullptr, nullptr, nullptr};
 
-    for (;;) {
-        unsigned long long w = 0;
-        if (lane == 0) w = atomicAdd(&a.ctrl->work, 1ULL);
-        w = __shfl_sync(0xffffffffu, w, 0);
+    const unsigned long long gw = (unsigned long long)blockIdx.x * kWarpsPerCta + warp;
+    for (bool first_item = true;; first_item = false) {
+        unsigned long long w = gw;
+        if (!first_item || gw >= q.n_static) {  // warp-uniform
+            if (lane == 0) w = q.n_static + atomicAdd(&a.ctrl->work, 1ULL);
+            w = __shfl_sync(0xffffffffu, w, 0);
+        }
         if (w >= q.n_items) break;
         long long i0;
         int cnt;
-        if (w < q.n_big) {
-            i0 = q.first + (long long)w * q.big;
-            cnt = q.big;
-        } else {
-            i0 = q.first + (long long)q.n_big * q.big + (long long)(w - q.n_big) * q.small;
-            cnt = q.small;
-        }
-        const long long left = q.first + q.count - i0;
-        if (left < cnt) cnt = (int)left;
+        queue_item(q, w, i0, cnt);
         if (lane < cnt) {
             const Hist hh = load_history(a.H, i0 + lane);
             setup_history(g, hh, s_state[lane]);
@@ -298,22 +406,20 @@ __global__ void __launch_bounds__(kThreads, 2) k_drop_block(const DropArgs a) {
             const PathState& S = s_state[p];
             const int K = S.K;
             if (K < 0) continue;  // skipped history: empty row (R7)
-            LaneRow<CMAX> row;
-            float dot, nrm;
+            float nrm;
             int nnz;
-            walk_history<CMAX, true, false>(g, S, s_tab, a.x, lane, row, dot, nrm, nnz, no_emit);
+            walk_history<false>(g, S, s_tab, lane, row, nrm, nnz, no_emit);
+            const int C = (K + 32) >> 5;
+            float dot = gather_row(row, lane, C, a.x);
             dot = warp_sum(dot);
             nrm = warp_sum(nrm);
             if (nrm > 0.0f) {  // non-empty row (R13)
                 const float r = __fdiv_rn(S.wepl - dot, nrm);
-#pragma unroll
-                for (int c = 0; c < CMAX; ++c) {
-                    if (c < row.C && row.lin[c] >= 0)
-                        atomicAdd(a.acc + row.lin[c], make_float2(r * row.len[c], ((row.heads >> c) & 1u) ? 1.0f : 0.0f));
-                }
+                scatter_row(row, lane, C, a.acc, r);
                 rows += (lane == 0);
                 nnz_total += nnz;
             }
+            __syncwarp();  // the row buffer is reused by the next history
             segs += (lane == 0) ? (K + 1) : 0;
         }
         __syncwarp();  // the state records are reused by the next item
@@ -326,30 +432,15 @@ __global__ void __launch_bounds__(kThreads, 2) k_drop_block(const DropArgs a) {
     }
 }
 
-// Chunk capacities the kernels are instantiated for: CMAX >= ceil((nmin + 1) / 32).
-#define PCT_FOR_CMAX(nmin, CALL)                  \
-    do {                                          \
-        const int cneed__ = ((nmin) + 32) >> 5;   \
-        if (cneed__ <= 3) { CALL(3); }            \
-        else if (cneed__ <= 5) { CALL(5); }       \
-        else if (cneed__ <= 7) { CALL(7); }       \
-        else if (cneed__ <= 9) { CALL(9); }       \
-        else if (cneed__ <= 16) { CALL(16); }     \
-        else { CALL(32); }                        \
-    } while (0)
-
 cudaError_t drop_configure(int nmin, int* grid_out) {
-    if (((nmin + 32) >> 5) > 32) return cudaErrorInvalidValue;
+    if (((nmin + 32) >> 5) > 64) return cudaErrorInvalidValue;
     const size_t smem = drop_smem_bytes(nmin);
     int dev = 0, sms = 0, per_sm = 0;
     cudaError_t e;
     if ((e = cudaGetDevice(&dev)) != cudaSuccess) return e;
     if ((e = cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev)) != cudaSuccess) return e;
-#define PCT_CFG(CM)                                                                                                  \
-    e = cudaFuncSetAttribute(k_drop_block<CM>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);               \
-    if (e == cudaSuccess) e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, k_drop_block<CM>, kThreads, smem)
-    PCT_FOR_CMAX(nmin, PCT_CFG);
-#undef PCT_CFG
+    e = cudaFuncSetAttribute(k_drop_block, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    if (e == cudaSuccess) e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, k_drop_block, kThreads, smem);
     if (e != cudaSuccess) return e;
     if (per_sm < 1) return cudaErrorLaunchOutOfResources;
     *grid_out = sms * per_sm;  // persistent: every CTA slot of the chip, work handed out dynamically
@@ -362,9 +453,7 @@ cudaError_t launch_drop_block(const DropArgs& a, int grid, cudaStream_t stream) 
     const long long need = (cnt + kWarpsPerCta - 1) / kWarpsPerCta;
     if (need < grid) grid = need < 1 ? 1 : (int)need;
     const size_t smem = drop_smem_bytes(a.g.nmin);
-#define PCT_LAUNCH(CM) k_drop_block<CM><<<grid, kThreads, smem, stream>>>(a)
-    PCT_FOR_CMAX(a.g.nmin, PCT_LAUNCH);
-#undef PCT_LAUNCH
+    k_drop_block<<<grid, kThreads, smem, stream>>>(a);
     return cudaGetLastError();
 }
 
@@ -450,13 +539,14 @@ cudaError_t launch_split_acc(float2* acc, float* delta, float* cnt, long long n,
 // the run heads and the non-zero count are those of the hot path; only the merged length of a
 // run (which the hot path never forms: it needs ||a_i||^2 and the unmerged scatter only) is
 // summed here, from the segment lengths just written.
-template <int CMAX>
 __global__ void __launch_bounds__(kThreads) k_rows(const RowsArgs a) {
     extern __shared__ __align__(16) unsigned char smem_raw[];
     const Geom g = a.g;
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    const SmemLayout lay = smem_layout(g.nmin);
     float4* s_tab = reinterpret_cast<float4*>(smem_raw);
-    PathState* s_state = reinterpret_cast<PathState*>(smem_raw + sizeof(float4) * tab_slots(g.nmin)) + warp * kBatch;
+    PathState* s_state = reinterpret_cast<PathState*>(smem_raw + lay.state_off) + warp * kBatch;
+    float2* row = reinterpret_cast<float2*>(smem_raw + lay.row_off) + warp * lay.row_slots;
     stage_table(s_tab, a.tab, g.nmin);
     for (long long r = (long long)blockIdx.x * kWarpsPerCta + warp; r < a.count; r += (long long)gridDim.x * kWarpsPerCta) {
         if (lane == 0) {
@@ -473,11 +563,17 @@ __global__ void __launch_bounds__(kThreads) k_rows(const RowsArgs a) {
             em.seg_len = a.seg_len ? a.seg_len + (size_t)r * a.max_seg : nullptr;
             em.row_len = a.row_len ? a.row_len + (size_t)r * a.max_seg : nullptr;
             em.nodes = a.nodes ? a.nodes + (size_t)r * (a.max_seg + 1) * 3 : nullptr;
-            LaneRow<CMAX> row;
-            float dot, nrm;
+            float nrm;
             int nnz;
-            walk_history<CMAX, false, true>(g, S, s_tab, nullptr, lane, row, dot, nrm, nnz, em);
+            walk_history<true>(g, S, s_tab, lane, row, nrm, nnz, em);
             nnz_total = __reduce_add_sync(0xffffffffu, nnz);
+            // the row as the hot path sees it: read back from the row buffer, segment-major
+            for (int k = lane; k <= K; k += 32) {
+                const float2 e = row[row_slot(k)];
+                if (em.seg_idx) em.seg_idx[k] = __float_as_int(e.x);
+                if (em.seg_len && __float_as_int(e.x) >= 0) em.seg_len[k] = fabsf(e.y);
+                if (em.row_len) em.row_len[k] = __float_as_int(e.y) < 0 ? 1.0f : 0.0f;
+            }
             __syncwarp();
             if (em.row_len && em.seg_idx && em.seg_len) {
                 for (int k = lane; k <= K; k += 32) {
@@ -499,17 +595,14 @@ __global__ void __launch_bounds__(kThreads) k_rows(const RowsArgs a) {
 }
 
 cudaError_t launch_rows(const RowsArgs& a, cudaStream_t stream) {
-    if (((a.g.nmin + 32) >> 5) > 32) return cudaErrorInvalidValue;
+    if (((a.g.nmin + 32) >> 5) > 64) return cudaErrorInvalidValue;
     const size_t smem = drop_smem_bytes(a.g.nmin);
     long long blocks = (a.count + kWarpsPerCta - 1) / kWarpsPerCta;
     if (blocks > 148 * 8) blocks = 148 * 8;
     if (blocks < 1) blocks = 1;
     cudaError_t e = cudaSuccess;
-#define PCT_ROWS(CM)                                                                                       \
-    e = cudaFuncSetAttribute(k_rows<CM>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);          \
-    if (e == cudaSuccess) k_rows<CM><<<(int)blocks, kThreads, smem, stream>>>(a)
-    PCT_FOR_CMAX(a.g.nmin, PCT_ROWS);
-#undef PCT_ROWS
+    e = cudaFuncSetAttribute(k_rows, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    if (e == cudaSuccess) k_rows<<<(int)blocks, kThreads, smem, stream>>>(a);
     if (e != cudaSuccess) return e;
     return cudaGetLastError();
 }

@@ -462,25 +462,51 @@ __device__ __forceinline__ float updated(float xv, float2 dc, float lambda) {
     return dc.y > 0.0f ? xv + __fdiv_rn(lambda * dc.x, dc.y) : xv;
 }
 
+#ifndef PCT_UPD_UNROLL
+#define PCT_UPD_UNROLL 2  // groups of four voxels a thread has in flight at once
+#endif
+#ifndef PCT_UPD_CTAS
+#define PCT_UPD_CTAS 8  // CTAs of 256 threads per SM
+#endif
+
+// One group = four consecutive voxels: two 128-bit accumulator loads, one 128-bit image load.  A
+// thread issues the loads of PCT_UPD_UNROLL groups (a CTA-stride apart, so that every load is
+// coalesced) before it touches any of them: the kernel is bound by L2 latency x bytes in flight.
 __global__ void __launch_bounds__(256) k_update(float* __restrict__ x, float2* __restrict__ acc, long long n_voxels,
                                                 float lambda, Ctrl* ctrl, long long n_blocks) {
+    constexpr int UN = PCT_UPD_UNROLL;
     const long long n4 = n_voxels >> 2;
     const long long stride = (long long)gridDim.x * blockDim.x;
     float4* x4 = reinterpret_cast<float4*>(x);
     float4* a4 = reinterpret_cast<float4*>(acc);
-    for (long long q = (long long)blockIdx.x * blockDim.x + threadIdx.x; q < n4; q += stride) {
-        const float4 a01 = a4[2 * q], a23 = a4[2 * q + 1];
-        const bool hit01 = a01.y > 0.0f || a01.w > 0.0f, hit23 = a23.y > 0.0f || a23.w > 0.0f;
-        if (hit01 || hit23) {
-            float4 xv = x4[q];
-            xv.x = updated(xv.x, make_float2(a01.x, a01.y), lambda);
-            xv.y = updated(xv.y, make_float2(a01.z, a01.w), lambda);
-            xv.z = updated(xv.z, make_float2(a23.x, a23.y), lambda);
-            xv.w = updated(xv.w, make_float2(a23.z, a23.w), lambda);
-            x4[q] = xv;
-            const float4 z = make_float4(0.f, 0.f, 0.f, 0.f);
-            if (hit01) a4[2 * q] = z;
-            if (hit23) a4[2 * q + 1] = z;
+    for (long long q0 = (long long)blockIdx.x * blockDim.x + threadIdx.x; q0 < n4; q0 += stride * UN) {
+        float4 a01[UN], a23[UN], xv[UN];
+#pragma unroll
+        for (int u = 0; u < UN; ++u) {
+            const long long q = q0 + u * stride;
+            if (q < n4) {
+                a01[u] = a4[2 * q];
+                a23[u] = a4[2 * q + 1];
+                xv[u] = x4[q];
+            } else {
+                a01[u] = a23[u] = xv[u] = make_float4(0.f, 0.f, 0.f, 0.f);
+            }
+        }
+#pragma unroll
+        for (int u = 0; u < UN; ++u) {
+            const long long q = q0 + u * stride;
+            const bool hit01 = a01[u].y > 0.0f || a01[u].w > 0.0f, hit23 = a23[u].y > 0.0f || a23[u].w > 0.0f;
+            if (hit01 || hit23) {  // (q < n4 is implied: out-of-range groups were loaded as zeros)
+                float4 v = xv[u];
+                v.x = updated(v.x, make_float2(a01[u].x, a01[u].y), lambda);
+                v.y = updated(v.y, make_float2(a01[u].z, a01[u].w), lambda);
+                v.z = updated(v.z, make_float2(a23[u].x, a23[u].y), lambda);
+                v.w = updated(v.w, make_float2(a23[u].z, a23[u].w), lambda);
+                x4[q] = v;
+                const float4 z = make_float4(0.f, 0.f, 0.f, 0.f);
+                if (hit01) a4[2 * q] = z;
+                if (hit23) a4[2 * q + 1] = z;
+            }
         }
     }
     if (blockIdx.x == 0) {
@@ -510,9 +536,9 @@ __global__ void __launch_bounds__(256) k_update(float* __restrict__ x, float2* _
 cudaError_t launch_update(float* x, float2* acc, long long n_voxels, float lambda, Ctrl* ctrl, long long n_blocks,
                           cudaStream_t stream) {
     const long long n4 = n_voxels >> 2;
-    long long blocks = (n4 + 255) / 256;
+    long long blocks = (n4 + 256 * PCT_UPD_UNROLL - 1) / (256 * PCT_UPD_UNROLL);
     if (blocks < 1) blocks = 1;
-    if (blocks > 148 * 16) blocks = 148 * 16;
+    if (blocks > 148 * PCT_UPD_CTAS) blocks = 148 * PCT_UPD_CTAS;
     k_update<<<(int)blocks, 256, 0, stream>>>(x, acc, n_voxels, lambda, ctrl, n_blocks);
     return cudaGetLastError();
 }

@@ -38,6 +38,9 @@ OPS_PER_SEGMENT = 106
 HBM_BYTES_PER_HISTORY = 38
 SM_COUNT = 148
 LANES_PER_SM = 128
+# dram__bytes_read.sum + dram__bytes_write.sum of ONE k_drop_block launch, from the committed
+# `ncu --set full` capture profiles/r1c_ncu_full.md (94.9 MB + 56.0 MB), keyed by (config, block size).
+NCU_DRAM_BYTES_PER_LAUNCH = {(3, 100000): 150.9e6}
 
 
 def parse_args():
@@ -324,7 +327,8 @@ def run_ours(args):
         "kernel_share_of_step": prof["accumulate_ms"] / prof["sweep_ms"],
         "update_kernel_ms": prof["update_ms"] / prof["blocks"],
         "timing": "CUDA events around every launch on the kernels' stream (pct_profile_sweep), one sweep of the timed workload",
-        "traffic": None,
+        "traffic": NCU_DRAM_BYTES_PER_LAUNCH.get((args.config, B)),
+        "traffic_source": "profiles/r1c_ncu_full.md (ncu --set full, bytes of DRAM per launch)",
         "hbm": {"achieved": hbm_ach, "peak": peaks["hbm_gbs"], "unit": "GB/s", "frac": hbm_ach / peaks["hbm_gbs"],
                 "peak_source": peaks["source"], "algorithmic": "38 B/history"},
         "l2_useful": {"achieved": l2_bytes / (k_ms * 1e-3) / 1e9, "unit": "GB/s",

@@ -241,6 +241,22 @@ def test_config1_sample(oracle_mod, pct, torch_cuda):
     _run_parity(oracle_mod, pct, torch_cuda, cfg, H, cfg.lam, cfg.block_size, 2)
 
 
+@pytest.mark.parametrize("index,n", [(3, 250_000), (4, 260_000)])
+def test_bench_launch_configuration_sample(oracle_mod, pct, torch_cuda, index, n):
+    """configs[3] / configs[4] geometry with THEIR block sizes (1e5 / 2e5 histories per launch: the
+    persistent grid, queue schedule and chunk sizes bench.py times), full blocks plus a ragged one,
+    two sweeps from a non-trivial image; every voxel compared with the oracle."""
+    import synth.cuda_gen as cuda_gen
+
+    cfg = synth.config(index)
+    D = cuda_gen.generate_cuda(cfg, n)  # the generator bench.py uses; ONE set of arrays feeds both sides
+    H = {k: v.cpu().numpy() for k, v in D.items()}
+    H["proj"] = H["proj"].view(np.uint16)
+    del D
+    x0 = synth.rsp_volume(cfg) * 0.8
+    _run_parity(oracle_mod, pct, torch_cuda, cfg, H, cfg.lam, cfg.block_size, 2, x0=x0)
+
+
 def test_graph_path_and_call_splitting(oracle_mod, pct, torch_cuda):
     """>= 128 (accumulate, update) pairs go through the replayed CUDA graph; one call with
     n_iter = 3 equals three calls with n_iter = 1 (the image is the whole solver state)."""

@@ -81,7 +81,10 @@ static void sigma1_inverse_table(float h32, int kmax, float4* out) {
         }
         const double gl = 1.0 + 0.038 * log(s / 361.0);
         const double W = gl * gl * (A * C - B * B);
-        out[k] = make_float4((float)(C / W), (float)(-B / W), (float)(A / W), 0.f);
+        // .w = s1 = float(k) * h, the ONE fp32 product of rule step 3b (identical to __fmul_rn(__int2float_rn(k), h)
+        // on the device: an exact int -> float conversion and one correctly rounded multiplication)
+        const volatile float s1 = (float)k * h32;
+        out[k] = make_float4((float)(C / W), (float)(-B / W), (float)(A / W), s1);
     }
 }
 

@@ -26,6 +26,10 @@ namespace pct {
 #ifndef PCT_BATCH
 #define PCT_BATCH 16
 #endif
+#ifndef PCT_WALK_UNROLL
+#define PCT_WALK_UNROLL 1
+#endif
+constexpr int kWalkUnroll = PCT_WALK_UNROLL;  // unroll factor of the walk loop
 constexpr int kWarpsPerCta = PCT_WARPS_PER_CTA;
 constexpr int kThreads = kWarpsPerCta * 32;
 constexpr int kCtasPerSm = PCT_CTAS_PER_SM;
@@ -176,7 +180,7 @@ __device__ __forceinline__ void walk_history(const Geom& g, const PathState& S, 
     prv.z = __shfl_up_sync(0xffffffffu, last.z, 1);
     if (lane == 0) prv = to_object(st, st.t0, st.u0, st.v0);  // node 0: the hull entry point (R9)
     MergeState m{-2, 0.0f, 0.0f, 0, 0, 0.0f};
-#pragma unroll 1
+#pragma unroll kWalkUnroll
     for (int c = 1; c < C; ++c) {
         const int k = k0 + c;  // node index; segment k-1 ends here
         float3 nd = mlp_node(g, st, s_tab[tab_slot(k)], k);

@@ -18,10 +18,10 @@
 namespace pct {
 
 #ifndef PCT_WARPS_PER_CTA
-#define PCT_WARPS_PER_CTA 8
+#define PCT_WARPS_PER_CTA 10
 #endif
 #ifndef PCT_CTAS_PER_SM
-#define PCT_CTAS_PER_SM 3  // register budget of k_drop_block: 65536 / (3 * 256) -> 80 per thread
+#define PCT_CTAS_PER_SM 2  // register budget of k_drop_block: 65536 / (2 * 320) -> 102 per thread (95 used)
 #endif
 #ifndef PCT_BATCH
 #define PCT_BATCH 16
@@ -51,7 +51,7 @@ struct SmemLayout {
 };
 __host__ __device__ inline SmemLayout smem_layout(int nmin) {
     SmemLayout l;
-    l.state_off = (int)sizeof(float4) * tab_slots(nmin);
+    l.state_off = 2 * (int)sizeof(float4) * tab_slots(nmin);  // paired table: two float4 arrays
     l.row_off = l.state_off + kWarpsPerCta * kBatch * (int)sizeof(PathState);
     l.row_slots = row_slots((nmin + 32) >> 5);  // K <= nmin: at most ceil((nmin + 1) / 32) segments per lane
     l.total = l.row_off + kWarpsPerCta * l.row_slots * (int)sizeof(float2);
@@ -84,11 +84,20 @@ __device__ __forceinline__ Hist load_history(const HistPtrs& H, long long i) {
     return hh;
 }
 
+// Paired layout: the walk evaluates nodes k and k+1 together (mlp_node2), so entry k holds the
+// functions of k and of k+1 side by side, ready as 64-bit register pairs:
+//   A[k] = (p11[k], p11[k+1], p12[k], p12[k+1])     at s_tab[tab_slot(k)]
+//   B[k] = (p22[k], p22[k+1], s1[k],  s1[k+1])      at s_tab[tab_slots(nmin) + tab_slot(k)]
 __device__ __forceinline__ void stage_table(float4* s_tab, const float4* __restrict__ tab, int nmin) {
     const int n = tab_slots(nmin);
-    for (int q = threadIdx.x; q < n; q += kThreads) s_tab[q] = make_float4(0.f, 0.f, 0.f, 0.f);
+    for (int q = threadIdx.x; q < 2 * n; q += kThreads) s_tab[q] = make_float4(0.f, 0.f, 0.f, 0.f);
     __syncthreads();
-    for (int k = threadIdx.x; k <= nmin; k += kThreads) s_tab[tab_slot(k)] = tab[k];
+    for (int k = threadIdx.x; k <= nmin; k += kThreads) {
+        const float4 a = tab[k];
+        const float4 b = k < nmin ? tab[k + 1] : make_float4(0.f, 0.f, 0.f, 0.f);
+        s_tab[tab_slot(k)] = make_float4(a.x, b.x, a.y, b.y);
+        s_tab[n + tab_slot(k)] = make_float4(a.z, b.z, a.w, b.w);
+    }
     __syncthreads();
 }
 
@@ -127,13 +136,10 @@ struct MergeState {
     float nrm;        // sum of squares of the FINISHED runs
 };
 
-// Segment `seg` of the lane, from node a to node b: voxel + length (rule step 4), merge, row-buffer entry.
+// Segment `seg` of the lane (it starts at node `a`), voxel and length known: merge, row-buffer entry.
 template <bool EMIT>
-__device__ __forceinline__ void take_segment(const Geom& g, const float3 a, const float3 b, int seg, int K, MergeState& m,
-                                             float2* row, const EmitPtrs& em) {
-    int lin;
-    float len;
-    segment(g, a, b, lin, len);
+__device__ __forceinline__ void take_segment(int lin, float len, const float3 a, int seg, int K, MergeState& m, float2* row,
+                                             const EmitPtrs& em) {
     const bool ok = (seg <= K) && lin >= 0;
     if (EMIT) {  // a dropped segment has no entry in the row; the inspection kernel still reports its length
         if (seg <= K && !ok && em.seg_len) em.seg_len[seg] = len;
@@ -156,39 +162,79 @@ __device__ __forceinline__ void take_segment(const Geom& g, const float3 a, cons
     }
 }
 
+__device__ __forceinline__ float3 lo3(const Node2& n) { return make_float3(lo_of(n.x), lo_of(n.y), lo_of(n.z)); }
+__device__ __forceinline__ float3 hi3(const Node2& n) { return make_float3(hi_of(n.x), hi_of(n.y), hi_of(n.z)); }
+__device__ __forceinline__ Node2 pair3(const float3 a, const float3 b) {
+    Node2 n;
+    n.x = pk(a.x, b.x);
+    n.y = pk(a.y, b.y);
+    n.z = pk(a.z, b.z);
+    return n;
+}
+
+// Nodes k and k+1 of the path (rule step 3), both halves of one packed evaluation; a node past the
+// last interior one is the hull exit point (R9).  k <= 0 gives an unspecified (unused) first half.
+__device__ __forceinline__ Node2 node_pair(const PathState& st, const float4* s_tab, const float4* s_tabB, int k, int K,
+                                           const float3 exitP) {
+    const int slot = tab_slot(k);
+    const Node2 n = mlp_node2(st, s_tab[slot], s_tabB[slot]);
+    float3 a = lo3(n), b = hi3(n);
+    if (k > K) a = exitP;
+    if (k + 1 > K) b = exitP;
+    return pair3(a, b);
+}
+
+// The two segments a.lo -> b.lo (segment `seg`) and a.hi -> b.hi (segment `seg` + 1): one packed
+// evaluation of rule step 4, then the sequential merge.  `first` = false skips the first of them.
+template <bool EMIT>
+__device__ __forceinline__ void take_two(const Geom& g, const Node2& a, const Node2& b, int seg, bool first, int K, MergeState& m,
+                                         float2* row, const EmitPtrs& em) {
+    f2 len, gx, gy, gz;
+    segment2(g, a, b, len, gx, gy, gz);
+    if (first) take_segment<EMIT>(voxel_of(g, lo_of(gx), lo_of(gy), lo_of(gz)), lo_of(len), lo3(a), seg, K, m, row, em);
+    take_segment<EMIT>(voxel_of(g, hi_of(gx), hi_of(gy), hi_of(gz)), hi_of(len), hi3(a), seg + 1, K, m, row, em);
+}
+
 // Walk of one history by one warp (steps 3-4 of the rule): fills the warp's row buffer, returns the
 // lane's part of ||a_i||^2 and of the non-zero count.
 //
-// Lane l owns segments k0 .. k0+C-1 (k0 = l*C), i.e. it needs nodes k0 .. k0+C.  It evaluates its
-// LAST node (k0+C) first and hands it to lane l+1 as that lane's start node with one shuffle (lane
-// 0 starts at the hull entry point), then walks nodes k0+1 .. k0+C-1 in a rolled loop -- the MLP
-// node at depth k*h is closed-form in k, there is no recurrence along the path.  Lanes past the end
-// of the path run the same instructions on harmless values and are masked.
+// Lane l owns segments k0 .. k0+C-1 (k0 = l*C), i.e. it needs nodes k0 .. k0+C.  Nodes are
+// evaluated two at a time (mlp_node2: packed fp32, one instruction for both).  The lane evaluates
+// its LAST two nodes (k0+C-1, k0+C) first and hands the last one to lane l+1 as that lane's start
+// node with one shuffle (lane 0 starts at the hull entry point), then walks the node pairs
+// (k0+1, k0+2), (k0+3, k0+4), ... -- two segments per trip -- up to node k0+C-2, and finishes with
+// the one or two segments that end at the nodes it evaluated first.  The MLP node at depth k*h is
+// closed-form in k, there is no recurrence along the path.  Lanes past the end of the path run the
+// same instructions on harmless values and are masked.
 template <bool EMIT>
 __device__ __forceinline__ void walk_history(const Geom& g, const PathState& S, const float4* s_tab, int lane, float2* row,
                                              float& nrm, int& nnz, const EmitPtrs& em) {
     const PathState st = S;  // shared memory -> registers, once per history
+    const float4* s_tabB = s_tab + tab_slots(g.nmin);
     const int K = st.K;
     const int C = (K + 32) >> 5;  // ceil((K + 1) / 32) segments per lane
     const int k0 = lane * C;
     const float3 exitP = to_object(st, st.t2, st.u2, st.v2);  // node K+1: the hull exit point, assigned (R9)
-    float3 last = mlp_node(g, st, s_tab[tab_slot(k0 + C)], k0 + C);
-    if (k0 + C > K) last = exitP;
+    const Node2 Z = node_pair(st, s_tab, s_tabB, k0 + C - 1, K, exitP);
+    const float3 last = hi3(Z);
     float3 prv;
     prv.x = __shfl_up_sync(0xffffffffu, last.x, 1);
     prv.y = __shfl_up_sync(0xffffffffu, last.y, 1);
     prv.z = __shfl_up_sync(0xffffffffu, last.z, 1);
     if (lane == 0) prv = to_object(st, st.t0, st.u0, st.v0);  // node 0: the hull entry point (R9)
     MergeState m{-2, 0.0f, 0.0f, 0, 0, 0.0f};
+    int c = 1;  // next node of the lane to evaluate; segments k0 .. k0+c-2 are done
 #pragma unroll kWalkUnroll
-    for (int c = 1; c < C; ++c) {
-        const int k = k0 + c;  // node index; segment k-1 ends here
-        float3 nd = mlp_node(g, st, s_tab[tab_slot(k)], k);
-        if (k > K) nd = exitP;
-        take_segment<EMIT>(g, prv, nd, k - 1, K, m, row, em);
-        prv = nd;
+    for (; c <= C - 2; c += 2) {
+        const Node2 N = node_pair(st, s_tab, s_tabB, k0 + c, K, exitP);
+        take_two<EMIT>(g, pair3(prv, lo3(N)), N, k0 + c - 1, true, K, m, row, em);
+        prv = hi3(N);
     }
-    take_segment<EMIT>(g, prv, last, k0 + C - 1, K, m, row, em);
+    {  // the last two segments (C - c + 1 == 2: via node k0+C-1) or the last one (prv IS node k0+C-1)
+        const bool two = C - c + 1 == 2;
+        const float3 mid = two ? lo3(Z) : prv;
+        take_two<EMIT>(g, pair3(prv, mid), pair3(mid, last), k0 + C - 2, two, K, m, row, em);
+    }
     if (EMIT) {
         if (k0 <= K && K < k0 + C) emit_node(em, K + 1, exitP);
     }

@@ -138,7 +138,7 @@ struct MergeState {
 
 // Segment `seg` of the lane (it starts at node `a`), voxel and length known: merge, row-buffer entry.
 template <bool EMIT>
-__device__ __forceinline__ void take_segment(int lin, float len, const float3 a, int seg, int K, MergeState& m, float2* row,
+__device__ __forceinline__ void take_segment(int lin, float len, const float3 a, int seg, int K, MergeState& m, unsigned row_sa,
                                              const EmitPtrs& em) {
     const bool ok = (seg <= K) && lin >= 0;
     if (EMIT) {  // a dropped segment has no entry in the row; the inspection kernel still reports its length
@@ -156,7 +156,9 @@ __device__ __forceinline__ void take_segment(int lin, float len, const float3 a,
     m.run_idx = lin;
     const bool head = fresh && lin >= 0;
     m.nnz += head ? 1 : 0;
-    row[row_slot(seg)] = make_float2(__int_as_float(lin), head ? -len : len);
+    // (an explicit 32-bit shared address: the compiler otherwise rebuilds the buffer's base in every trip)
+    asm volatile("st.shared.v2.b32 [%0], {%1, %2};" ::"r"(row_sa + 8u * (unsigned)row_slot(seg)), "r"(lin),
+                 "r"(__float_as_int(head ? -len : len)) : "memory");
     if (EMIT) {
         if (seg <= K) emit_node(em, seg, a);
     }
@@ -188,11 +190,11 @@ __device__ __forceinline__ Node2 node_pair(const PathState& st, const float4* s_
 // evaluation of rule step 4, then the sequential merge.  `first` = false skips the first of them.
 template <bool EMIT>
 __device__ __forceinline__ void take_two(const Geom& g, const Node2& a, const Node2& b, int seg, bool first, int K, MergeState& m,
-                                         float2* row, const EmitPtrs& em) {
+                                         unsigned row_sa, const EmitPtrs& em) {
     f2 len, gx, gy, gz;
     segment2(g, a, b, len, gx, gy, gz);
-    if (first) take_segment<EMIT>(voxel_of(g, lo_of(gx), lo_of(gy), lo_of(gz)), lo_of(len), lo3(a), seg, K, m, row, em);
-    take_segment<EMIT>(voxel_of(g, hi_of(gx), hi_of(gy), hi_of(gz)), hi_of(len), hi3(a), seg + 1, K, m, row, em);
+    if (first) take_segment<EMIT>(voxel_of(g, lo_of(gx), lo_of(gy), lo_of(gz)), lo_of(len), lo3(a), seg, K, m, row_sa, em);
+    take_segment<EMIT>(voxel_of(g, hi_of(gx), hi_of(gy), hi_of(gz)), hi_of(len), hi3(a), seg + 1, K, m, row_sa, em);
 }
 
 // Walk of one history by one warp (steps 3-4 of the rule): fills the warp's row buffer, returns the
@@ -223,17 +225,18 @@ __device__ __forceinline__ void walk_history(const Geom& g, const PathState& S, 
     prv.z = __shfl_up_sync(0xffffffffu, last.z, 1);
     if (lane == 0) prv = to_object(st, st.t0, st.u0, st.v0);  // node 0: the hull entry point (R9)
     MergeState m{-2, 0.0f, 0.0f, 0, 0, 0.0f};
+    const unsigned row_sa = (unsigned)__cvta_generic_to_shared(row);
     int c = 1;  // next node of the lane to evaluate; segments k0 .. k0+c-2 are done
 #pragma unroll kWalkUnroll
     for (; c <= C - 2; c += 2) {
         const Node2 N = node_pair(st, s_tab, s_tabB, k0 + c, K, exitP);
-        take_two<EMIT>(g, pair3(prv, lo3(N)), N, k0 + c - 1, true, K, m, row, em);
+        take_two<EMIT>(g, pair3(prv, lo3(N)), N, k0 + c - 1, true, K, m, row_sa, em);
         prv = hi3(N);
     }
     {  // the last two segments (C - c + 1 == 2: via node k0+C-1) or the last one (prv IS node k0+C-1)
         const bool two = C - c + 1 == 2;
         const float3 mid = two ? lo3(Z) : prv;
-        take_two<EMIT>(g, pair3(prv, mid), pair3(mid, last), k0 + C - 2, two, K, m, row, em);
+        take_two<EMIT>(g, pair3(prv, mid), pair3(mid, last), k0 + C - 2, two, K, m, row_sa, em);
     }
     if (EMIT) {
         if (k0 <= K && K < k0 + C) emit_node(em, K + 1, exitP);

@@ -26,6 +26,9 @@ namespace pct {
 #ifndef PCT_BATCH
 #define PCT_BATCH 16
 #endif
+#ifndef PCT_ACC_EVICT_FIRST
+#define PCT_ACC_EVICT_FIRST 1  // accumulator traffic of k_update carries an L2 evict_first policy
+#endif
 #ifndef PCT_WALK_UNROLL
 #define PCT_WALK_UNROLL 1
 #endif
@@ -290,17 +293,39 @@ __device__ __forceinline__ void red_add_v2(float2* acc, int lin, float v, float 
         :: "l"(acc), "r"(lin), "f"(v), "f"(cnt) : "memory");
 }
 
+// L2 residency.  The image (4 B/voxel) and the accumulator (8 B/voxel) together do not stay in the
+// L2 across the two kernels of a DROP block (100 MB at 256 x 256 x 128 against 126 MB split over two
+// dies), so both kernels kept re-reading them from HBM and one gather in three paid the DRAM latency.
+// Every access to the IMAGE carries an evict_last policy, the accumulator traffic stays evict_normal:
+// the image stays resident, the gather always hits the L2.
+__device__ __forceinline__ unsigned long long policy_evict_last() {
+    unsigned long long pol;
+    asm("createpolicy.fractional.L2::evict_last.b64 %0, 1.0;" : "=l"(pol));
+    return pol;
+}
+__device__ __forceinline__ unsigned long long policy_evict_first() {
+    unsigned long long pol;
+    asm("createpolicy.fractional.L2::evict_first.b64 %0, 1.0;" : "=l"(pol));
+    return pol;
+}
+__device__ __forceinline__ float ld_image(const float* p, unsigned long long pol) {
+    float v;
+    asm volatile("ld.global.nc.L2::cache_hint.f32 %0, [%1], %2;" : "=f"(v) : "l"(p), "l"(pol));
+    return v;
+}
+
 template <int N>
 __device__ __forceinline__ float gather_n(const float2* rl, const float* __restrict__ x) {
     float2 e[N];
     float xv[N];
+    const unsigned long long pol = policy_evict_last();
 #pragma unroll
     for (int u = 0; u < N; ++u) e[u] = rl[33 * u];
 #pragma unroll
     for (int u = 0; u < N; ++u) {
         const int lin = __float_as_int(e[u].x);
         xv[u] = 0.0f;
-        if (lin >= 0) xv[u] = __ldg(x + lin);
+        if (lin >= 0) xv[u] = ld_image(x + lin, pol);
     }
     float dot = 0.0f;
 #pragma unroll
@@ -522,12 +547,30 @@ __device__ __forceinline__ float updated(float xv, float2 dc, float lambda) {
 #define PCT_UPD_CTAS 8  // CTAs of 256 threads per SM
 #endif
 
+__device__ __forceinline__ float4 ld4_hint(const float4* p, unsigned long long pol) {
+    float4 v;
+    asm volatile("ld.global.L2::cache_hint.v4.f32 {%0, %1, %2, %3}, [%4], %5;"
+                 : "=f"(v.x), "=f"(v.y), "=f"(v.z), "=f"(v.w) : "l"(p), "l"(pol) : "memory");
+    return v;
+}
+__device__ __forceinline__ void st4_hint(float4* p, float4 v, unsigned long long pol) {
+    asm volatile("st.global.L2::cache_hint.v4.f32 [%0], {%1, %2, %3, %4}, %5;"
+                 :: "l"(p), "f"(v.x), "f"(v.y), "f"(v.z), "f"(v.w), "l"(pol) : "memory");
+}
+
 // One group = four consecutive voxels: two 128-bit accumulator loads, one 128-bit image load.  A
 // thread issues the loads of PCT_UPD_UNROLL groups (a CTA-stride apart, so that every load is
 // coalesced) before it touches any of them: the kernel is bound by L2 latency x bytes in flight.
 __global__ void __launch_bounds__(256) k_update(float* __restrict__ x, float2* __restrict__ acc, long long n_voxels,
                                                 float lambda, Ctrl* ctrl, long long n_blocks) {
     constexpr int UN = PCT_UPD_UNROLL;
+    const unsigned long long keep = policy_evict_last();
+#if PCT_ACC_EVICT_FIRST
+    const unsigned long long stream_pol = policy_evict_first();
+#define PCT_LD_ACC(p) ld4_hint(p, stream_pol)
+#else
+#define PCT_LD_ACC(p) (*(p))
+#endif
     const long long n4 = n_voxels >> 2;
     const long long stride = (long long)gridDim.x * blockDim.x;
     float4* x4 = reinterpret_cast<float4*>(x);
@@ -538,9 +581,9 @@ __global__ void __launch_bounds__(256) k_update(float* __restrict__ x, float2* _
         for (int u = 0; u < UN; ++u) {
             const long long q = q0 + u * stride;
             if (q < n4) {
-                a01[u] = a4[2 * q];
-                a23[u] = a4[2 * q + 1];
-                xv[u] = x4[q];
+                a01[u] = PCT_LD_ACC(a4 + 2 * q);
+                a23[u] = PCT_LD_ACC(a4 + 2 * q + 1);
+                xv[u] = ld4_hint(x4 + q, keep);
             } else {
                 a01[u] = a23[u] = xv[u] = make_float4(0.f, 0.f, 0.f, 0.f);
             }
@@ -555,9 +598,9 @@ __global__ void __launch_bounds__(256) k_update(float* __restrict__ x, float2* _
                 v.y = updated(v.y, make_float2(a01[u].z, a01[u].w), lambda);
                 v.z = updated(v.z, make_float2(a23[u].x, a23[u].y), lambda);
                 v.w = updated(v.w, make_float2(a23[u].z, a23[u].w), lambda);
-                x4[q] = v;
+                st4_hint(x4 + q, v, keep);
                 const float4 z = make_float4(0.f, 0.f, 0.f, 0.f);
-                if (hit01) a4[2 * q] = z;
+                if (hit01) a4[2 * q] = z;  // (hinting these stores, or the reductions, measured no better)
                 if (hit23) a4[2 * q + 1] = z;
             }
         }

@@ -38,10 +38,14 @@ constexpr int kThreads = kWarpsPerCta * 32;
 constexpr int kCtasPerSm = PCT_CTAS_PER_SM;
 constexpr int kBatch = PCT_BATCH;  // histories a warp takes from the work queue per trip (at most)
 
-// Sigma1^-1 table in shared memory: entry k sits at slot k + (k >> 3), so that the 8 lanes of a
-// quarter warp, which read entries C apart, fall into different 16-byte bank groups for every
-// chunk size C <= 9 (plain layout: C = 8 would be an 8-way conflict).  The table is padded with
-// zero entries up to k = nmin + 32: lanes past the end of a path read (and discard) them.
+// Sigma1^-1 table in shared memory.  Lane l reads the entries of nodes l*C + c: 32 entries C apart per
+// 128-bit load, four wavefronts of eight lanes at best.  In a plain layout that best case holds for
+// every ODD chunk size C and fails for even ones (C = 8: all lanes in one bank group, 32 wavefronts);
+// with entry k at slot k + (k >> 3) it holds for C = 8 (and is fair for the other even sizes) but
+// C = 7 degenerates to 24 wavefronts.  No single layout serves both, and C = 7 and C = 8 are two
+// thirds of all histories at 256 x 256 x 128, so the table is staged TWICE -- plain and padded -- and a
+// history picks its copy by the parity of its C (warp-uniform).  Both copies are padded with zero
+// entries up to k = nmin + 33: lanes past the end of a path read (and discard) them.
 __host__ __device__ inline int tab_slot(int k) { return k + (k >> 3); }
 __host__ __device__ inline int tab_slots(int nmin) { return (tab_slot(nmin + 33) + 4) & ~3; }
 
@@ -54,7 +58,7 @@ struct SmemLayout {
 };
 __host__ __device__ inline SmemLayout smem_layout(int nmin) {
     SmemLayout l;
-    l.state_off = 2 * (int)sizeof(float4) * tab_slots(nmin);  // paired table: two float4 arrays
+    l.state_off = 4 * (int)sizeof(float4) * tab_slots(nmin);  // two copies of the paired table (two float4 arrays each)
     l.row_off = l.state_off + kWarpsPerCta * kBatch * (int)sizeof(PathState);
     l.row_slots = row_slots((nmin + 32) >> 5);  // K <= nmin: at most ceil((nmin + 1) / 32) segments per lane
     l.total = l.row_off + kWarpsPerCta * l.row_slots * (int)sizeof(float2);
@@ -89,17 +93,20 @@ __device__ __forceinline__ Hist load_history(const HistPtrs& H, long long i) {
 
 // Paired layout: the walk evaluates nodes k and k+1 together (mlp_node2), so entry k holds the
 // functions of k and of k+1 side by side, ready as 64-bit register pairs:
-//   A[k] = (p11[k], p11[k+1], p12[k], p12[k+1])     at s_tab[tab_slot(k)]
-//   B[k] = (p22[k], p22[k+1], s1[k],  s1[k+1])      at s_tab[tab_slots(nmin) + tab_slot(k)]
+//   A[k] = (p11[k], p11[k+1], p12[k], p12[k+1]),  B[k] = (p22[k], p22[k+1], s1[k], s1[k+1]).
+// s_tab = | A padded | B padded | A plain | B plain |, each of n = tab_slots(nmin) entries.
 __device__ __forceinline__ void stage_table(float4* s_tab, const float4* __restrict__ tab, int nmin) {
     const int n = tab_slots(nmin);
-    for (int q = threadIdx.x; q < 2 * n; q += kThreads) s_tab[q] = make_float4(0.f, 0.f, 0.f, 0.f);
+    for (int q = threadIdx.x; q < 4 * n; q += kThreads) s_tab[q] = make_float4(0.f, 0.f, 0.f, 0.f);
     __syncthreads();
     for (int k = threadIdx.x; k <= nmin; k += kThreads) {
         const float4 a = tab[k];
         const float4 b = k < nmin ? tab[k + 1] : make_float4(0.f, 0.f, 0.f, 0.f);
-        s_tab[tab_slot(k)] = make_float4(a.x, b.x, a.y, b.y);
-        s_tab[n + tab_slot(k)] = make_float4(a.z, b.z, a.w, b.w);
+        const float4 A = make_float4(a.x, b.x, a.y, b.y), B = make_float4(a.z, b.z, a.w, b.w);
+        s_tab[tab_slot(k)] = A;
+        s_tab[n + tab_slot(k)] = B;
+        s_tab[2 * n + k] = A;
+        s_tab[3 * n + k] = B;
     }
     __syncthreads();
 }
@@ -179,9 +186,9 @@ __device__ __forceinline__ Node2 pair3(const float3 a, const float3 b) {
 
 // Nodes k and k+1 of the path (rule step 3), both halves of one packed evaluation; a node past the
 // last interior one is the hull exit point (R9).  k <= 0 gives an unspecified (unused) first half.
-__device__ __forceinline__ Node2 node_pair(const PathState& st, const float4* s_tab, const float4* s_tabB, int k, int K,
-                                           const float3 exitP) {
-    const int slot = tab_slot(k);
+__device__ __forceinline__ Node2 node_pair(const PathState& st, const float4* s_tab, const float4* s_tabB, int pad_mask, int k,
+                                           int K, const float3 exitP) {
+    const int slot = k + ((k >> 3) & pad_mask);  // padded copy: tab_slot(k); plain copy: k
     const Node2 n = mlp_node2(st, s_tab[slot], s_tabB[slot]);
     float3 a = lo3(n), b = hi3(n);
     if (k > K) a = exitP;
@@ -215,12 +222,15 @@ template <bool EMIT>
 __device__ __forceinline__ void walk_history(const Geom& g, const PathState& S, const float4* s_tab, int lane, float2* row,
                                              float& nrm, int& nnz, const EmitPtrs& em) {
     const PathState st = S;  // shared memory -> registers, once per history
-    const float4* s_tabB = s_tab + tab_slots(g.nmin);
     const int K = st.K;
     const int C = (K + 32) >> 5;  // ceil((K + 1) / 32) segments per lane
+    const int tab_n = tab_slots(g.nmin);
+    const int pad_mask = (C & 1) ? 0 : -1;  // odd C: the plain copy of the table, even C: the padded one
+    const float4* s_tabA = s_tab + ((C & 1) ? 2 * tab_n : 0);
+    const float4* s_tabB = s_tabA + tab_n;
     const int k0 = lane * C;
     const float3 exitP = to_object(st, st.t2, st.u2, st.v2);  // node K+1: the hull exit point, assigned (R9)
-    const Node2 Z = node_pair(st, s_tab, s_tabB, k0 + C - 1, K, exitP);
+    const Node2 Z = node_pair(st, s_tabA, s_tabB, pad_mask, k0 + C - 1, K, exitP);
     const float3 last = hi3(Z);
     float3 prv;
     prv.x = __shfl_up_sync(0xffffffffu, last.x, 1);
@@ -232,7 +242,7 @@ __device__ __forceinline__ void walk_history(const Geom& g, const PathState& S, 
     int c = 1;  // next node of the lane to evaluate; segments k0 .. k0+c-2 are done
 #pragma unroll kWalkUnroll
     for (; c <= C - 2; c += 2) {
-        const Node2 N = node_pair(st, s_tab, s_tabB, k0 + c, K, exitP);
+        const Node2 N = node_pair(st, s_tabA, s_tabB, pad_mask, k0 + c, K, exitP);
         take_two<EMIT>(g, pair3(prv, lo3(N)), N, k0 + c - 1, true, K, m, row_sa, em);
         prv = hi3(N);
     }

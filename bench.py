@@ -39,8 +39,10 @@ HBM_BYTES_PER_HISTORY = 38
 SM_COUNT = 148
 LANES_PER_SM = 128
 # dram__bytes_read.sum + dram__bytes_write.sum of ONE k_drop_block launch, from the committed
-# `ncu --set full` capture profiles/r1c_ncu_full.md (94.9 MB + 56.0 MB), keyed by (config, block size).
-NCU_DRAM_BYTES_PER_LAUNCH = {(3, 100000): 150.9e6}
+# `ncu --set full` capture profiles/r1d_ncu_full.md (95.0 MB + 57.1 MB; ncu flushes the caches before the
+# replay), keyed by (config, block size); the same launch with warm caches (profiles/r1d_dram_warm.md).
+NCU_DRAM_BYTES_PER_LAUNCH = {(3, 100000): 152.1e6}
+NCU_DRAM_BYTES_PER_LAUNCH_WARM = {(3, 100000): 145.6e6}
 
 
 def parse_args():
@@ -328,7 +330,9 @@ def run_ours(args):
         "update_kernel_ms": prof["update_ms"] / prof["blocks"],
         "timing": "CUDA events around every launch on the kernels' stream (pct_profile_sweep), one sweep of the timed workload",
         "traffic": NCU_DRAM_BYTES_PER_LAUNCH.get((args.config, B)),
-        "traffic_source": "profiles/r1c_ncu_full.md (ncu --set full, bytes of DRAM per launch)",
+        "traffic_source": "profiles/r1d_ncu_full.md (ncu --set full, bytes of DRAM per launch, caches flushed by ncu)",
+        "traffic_warm": NCU_DRAM_BYTES_PER_LAUNCH_WARM.get((args.config, B)),
+        "traffic_warm_source": "profiles/r1d_dram_warm.md (ncu --cache-control none)",
         "hbm": {"achieved": hbm_ach, "peak": peaks["hbm_gbs"], "unit": "GB/s", "frac": hbm_ach / peaks["hbm_gbs"],
                 "peak_source": peaks["source"], "algorithmic": "38 B/history"},
         "l2_useful": {"achieved": l2_bytes / (k_ms * 1e-3) / 1e9, "unit": "GB/s",

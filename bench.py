@@ -204,16 +204,13 @@ def run_ours(args):
     if world > 1:
         dist.init_process_group("nccl", device_id=torch.device("cuda", local))
 
+    from paper_1707_05014_b200 import replicas
+
     def barrier():
-        if world > 1:
-            dist.barrier()
+        replicas.barrier(world)
 
     def max_over_ranks(v):
-        if world == 1:
-            return v
-        t = torch.tensor([v], dtype=torch.float64, device="cuda")
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        return float(t.item())
+        return replicas.max_over_ranks(v, world, "cuda")
 
     cfg = synth.config(args.config)
     n = cfg.n if args.histories is None else int(args.histories)
@@ -221,7 +218,7 @@ def run_ours(args):
     n_blocks = (n + B - 1) // B
 
     # replicas only: rank r draws histories [r*n, (r+1)*n) of the same seeded stream
-    D = cuda_gen.generate_cuda(cfg, n, first=rank * n)
+    D = cuda_gen.generate_cuda(cfg, n, first=replicas.shard_first(rank, n))
     P = synth.to_pct_names(D)
     stream = torch.cuda.Stream()
     out = {}
@@ -242,9 +239,8 @@ def run_ours(args):
                 e1.record()
                 torch.cuda.synchronize()
                 barrier()
-            ms = max_over_ranks(e0.elapsed_time(e1))
+            ms, out["value"] = replicas.whole_job_rate(e0.elapsed_time(e1), n, args.steps, world, "cuda")
             out["ms_per_step"] = ms / args.steps
-            out["value"] = world * n * args.steps / (ms * 1e-3)
             out["clocks"] = clk.summary()
             out["stats"] = pct.pct_get_stats(ctx)
             # the dominant kernel, CUDA events around every launch, one more sweep of the same workload

@@ -7,6 +7,7 @@
 #include <string.h>
 
 #include <new>
+#include <vector>
 
 #include "../../include/pct.h"
 #include "pct_internal.h"
@@ -29,6 +30,15 @@ struct pct_ctx {
     HistPtrs H{};
     float* tables = nullptr;  // owned: pcos | psin
     void* owned_hist = nullptr;  // owned device block of the host entry point
+    // pipelined upload of the host entry point: chunks of 2^20 .. 2^24 histories go up on a copy
+    // stream of their own, one event per chunk; the compute stream waits for a chunk only when a
+    // DROP block (or an inspection call) first needs it, so the first sweep overlaps the upload
+    cudaStream_t copy_stream = nullptr;
+    std::vector<cudaEvent_t> chunk_ev;
+    std::vector<long long> chunk_end;  // chunk i holds histories [chunk_end[i-1], chunk_end[i])
+    size_t chunks_waited = 0;  // events [0, chunks_waited) are already ordered before c->stream's tail
+    long long owned_n = 0;     // histories the owned block was sized for (reused by the next upload of the same size)
+    int owned_n_proj = 0;
     // cached CUDA graph of kGraphPairs (accumulate, update) pairs
     cudaGraphExec_t graph = nullptr;
     float graph_lambda = 0.f;
@@ -40,6 +50,11 @@ struct pct_ctx {
 
 static thread_local char g_create_err[512] = {0};
 static const int kGraphPairs = 64;
+// Upload chunks (histories): the first one is small so that the first DROP blocks start after about a
+// millisecond, the following ones double up to 2^24 (64 MB per float field) so that a 19 GB upload is
+// a few hundred copy calls -- more would overflow the copy stream's submission queue and block the
+// host inside pct_set_histories_host while the compute stream sits idle.
+static const long long kUploadChunkMin = 1LL << 20, kUploadChunkMax = 1LL << 24;
 
 static int fail(pct_ctx* c, int code, const char* fmt, const char* detail = "") {
     char* dst = c ? c->err : g_create_err;
@@ -95,11 +110,29 @@ static void drop_graph(pct_ctx* c) {
     }
 }
 
+// Make the compute stream wait for the upload of histories [0, upto) (all of them: upto < 0).
+static int wait_upload(pct_ctx* c, long long upto) {
+    const size_t all = c->chunk_ev.size();
+    while (c->chunks_waited < all && (upto < 0 || c->chunks_waited == 0 || c->chunk_end[c->chunks_waited - 1] < upto)) {
+        CUDA_TRY(c, cudaStreamWaitEvent(c->stream, c->chunk_ev[c->chunks_waited], 0));
+        ++c->chunks_waited;
+    }
+    return PCT_OK;
+}
+
 static void release_histories(pct_ctx* c) {
     drop_graph(c);
+    if (!c->chunk_ev.empty()) {
+        if (c->copy_stream) cudaStreamSynchronize(c->copy_stream);
+        for (cudaEvent_t e : c->chunk_ev) cudaEventDestroy(e);
+        c->chunk_ev.clear();
+    }
+    c->chunk_end.clear();
+    c->chunks_waited = 0;
     if (c->owned_hist) cudaFree(c->owned_hist);
     if (c->tables) cudaFree(c->tables);
     c->owned_hist = nullptr;
+    c->owned_n = 0;
     c->tables = nullptr;
     c->have_hist = false;
     c->n = 0;
@@ -172,6 +205,7 @@ extern "C" void pct_destroy(pct_ctx* c) {
     if (!c) return;
     cudaStreamSynchronize(c->stream);
     release_histories(c);
+    if (c->copy_stream) cudaStreamDestroy(c->copy_stream);
     if (c->x) cudaFree(c->x);
     if (c->acc) cudaFree(c->acc);
     if (c->tab) cudaFree(c->tab);
@@ -222,23 +256,52 @@ extern "C" int pct_set_histories(pct_ctx* c, int64_t n, const pct_histories* h) 
 extern "C" int pct_set_histories_host(pct_ctx* c, int64_t n, const pct_histories* h) {
     int rc = check_histories(c, n, h, false);
     if (rc) return rc;
-    release_histories(c);
     // one owned block: 9 float arrays (each padded to 256 B) + the uint16 array
     const size_t fa = ((sizeof(float) * (size_t)n + 255) / 256) * 256;
     const size_t total = 9 * fa + ((sizeof(uint16_t) * (size_t)n + 255) / 256) * 256;
-    CUDA_TRY(c, cudaMalloc(&c->owned_hist, total));
-    CUDA_TRY(c, cudaMalloc(&c->tables, sizeof(float) * 2 * h->n_proj));
-    const float* src[9] = {h->entry_t, h->entry_v, h->exit_t, h->exit_v, h->entry_dt, h->entry_dv, h->exit_dt, h->exit_dv, h->wepl};
-    const float* dst[9];
-    for (int i = 0; i < 9; ++i) {
-        float* d = (float*)((char*)c->owned_hist + i * fa);
-        dst[i] = d;
-        CUDA_TRY(c, cudaMemcpyAsync(d, src[i], sizeof(float) * (size_t)n, cudaMemcpyHostToDevice, c->stream));
+    if (c->owned_hist && c->tables && c->owned_n == n && c->owned_n_proj == h->n_proj) {
+        // a new set of the same size (the next acquisition through the same pipeline): the device block,
+        // the tables and the cached graph are reused -- no 19 GB cudaFree + cudaMalloc per upload.  The
+        // new upload is ordered after everything already enqueued that reads the old histories.
+        if (c->copy_stream) CUDA_TRY(c, cudaStreamSynchronize(c->copy_stream));
+        for (cudaEvent_t e : c->chunk_ev) cudaEventDestroy(e);
+        c->chunk_ev.clear();
+        c->chunk_end.clear();
+        c->chunks_waited = 0;
+        cudaEvent_t tail = nullptr;
+        CUDA_TRY(c, cudaEventCreateWithFlags(&tail, cudaEventDisableTiming));
+        cudaError_t e = cudaEventRecord(tail, c->stream);
+        if (!c->copy_stream && e == cudaSuccess) e = cudaStreamCreateWithFlags(&c->copy_stream, cudaStreamNonBlocking);
+        if (e == cudaSuccess) e = cudaStreamWaitEvent(c->copy_stream, tail, 0);
+        cudaEventDestroy(tail);
+        CUDA_TRY(c, e);
+    } else {
+        release_histories(c);
+        CUDA_TRY(c, cudaMalloc(&c->owned_hist, total));
+        CUDA_TRY(c, cudaMalloc(&c->tables, sizeof(float) * 2 * h->n_proj));
+        c->owned_n = n;
+        c->owned_n_proj = h->n_proj;
     }
+    const float* src[9] = {h->entry_t, h->entry_v, h->exit_t, h->exit_v, h->entry_dt, h->entry_dv, h->exit_dt, h->exit_dv, h->wepl};
+    float* dst[9];
+    for (int i = 0; i < 9; ++i) dst[i] = (float*)((char*)c->owned_hist + i * fa);
     uint16_t* dproj = (uint16_t*)((char*)c->owned_hist + 9 * fa);
-    CUDA_TRY(c, cudaMemcpyAsync(dproj, h->proj, sizeof(uint16_t) * (size_t)n, cudaMemcpyHostToDevice, c->stream));
-    CUDA_TRY(c, cudaMemcpyAsync(c->tables, h->proj_cos, sizeof(float) * h->n_proj, cudaMemcpyHostToDevice, c->stream));
-    CUDA_TRY(c, cudaMemcpyAsync(c->tables + h->n_proj, h->proj_sin, sizeof(float) * h->n_proj, cudaMemcpyHostToDevice, c->stream));
+    if (!c->copy_stream) CUDA_TRY(c, cudaStreamCreateWithFlags(&c->copy_stream, cudaStreamNonBlocking));
+    // chunk by chunk, all ten fields of a chunk together, one event per chunk (the tables ride with chunk 0)
+    CUDA_TRY(c, cudaMemcpyAsync(c->tables, h->proj_cos, sizeof(float) * h->n_proj, cudaMemcpyHostToDevice, c->copy_stream));
+    CUDA_TRY(c, cudaMemcpyAsync(c->tables + h->n_proj, h->proj_sin, sizeof(float) * h->n_proj, cudaMemcpyHostToDevice, c->copy_stream));
+    long long chunk = kUploadChunkMin;
+    for (long long i0 = 0; i0 < n; i0 += chunk, chunk = chunk < kUploadChunkMax && i0 >= 2 * kUploadChunkMin ? 2 * chunk : chunk) {
+        const size_t cnt = (size_t)(n - i0 < chunk ? n - i0 : chunk);
+        for (int i = 0; i < 9; ++i)
+            CUDA_TRY(c, cudaMemcpyAsync(dst[i] + i0, src[i] + i0, sizeof(float) * cnt, cudaMemcpyHostToDevice, c->copy_stream));
+        CUDA_TRY(c, cudaMemcpyAsync(dproj + i0, h->proj + i0, sizeof(uint16_t) * cnt, cudaMemcpyHostToDevice, c->copy_stream));
+        cudaEvent_t ev = nullptr;
+        CUDA_TRY(c, cudaEventCreateWithFlags(&ev, cudaEventDisableTiming));
+        c->chunk_ev.push_back(ev);
+        c->chunk_end.push_back(i0 + (long long)cnt);
+        CUDA_TRY(c, cudaEventRecord(ev, c->copy_stream));
+    }
     c->H = HistPtrs{dst[0], dst[1], dst[2], dst[3], dst[4], dst[5], dst[6], dst[7], dst[8], dproj,
                     c->tables, c->tables + h->n_proj, h->n_proj};
     c->n = n;
@@ -303,10 +366,16 @@ extern "C" int pct_iterate(pct_ctx* c, float lambda, int64_t block_size, int n_i
             c->graph_n = c->n;
             c->graph_hist_key = (const void*)c->H.t_in;
         }
-        for (; done + kGraphPairs <= pairs; done += kGraphPairs) CUDA_TRY(c, cudaGraphLaunch(c->graph, c->stream));
+        for (; done + kGraphPairs <= pairs; done += kGraphPairs) {
+            // blocks done .. done+63 of the first sweep need the histories below (done + 64) * block_size
+            int rc = wait_upload(c, done + kGraphPairs <= n_blocks ? (done + kGraphPairs) * block_size : -1);
+            if (rc) return rc;
+            CUDA_TRY(c, cudaGraphLaunch(c->graph, c->stream));
+        }
     }
     for (; done < pairs; ++done) {
-        int rc = enqueue_pair(c, a, lambda, n_blocks, c->stream);
+        int rc = wait_upload(c, done < n_blocks ? (done + 1) * block_size : -1);
+        if (rc == PCT_OK) rc = enqueue_pair(c, a, lambda, n_blocks, c->stream);
         if (rc) return rc;
     }
     return PCT_OK;
@@ -314,6 +383,7 @@ extern "C" int pct_iterate(pct_ctx* c, float lambda, int64_t block_size, int n_i
 
 extern "C" int pct_synchronize(pct_ctx* c) {
     if (!c) return PCT_EINVAL;
+    if (int rc = wait_upload(c, -1)) return rc;  // the host arrays are free once this returns
     CUDA_TRY(c, cudaStreamSynchronize(c->stream));
     return PCT_OK;
 }
@@ -321,6 +391,7 @@ extern "C" int pct_synchronize(pct_ctx* c) {
 extern "C" int pct_get_image(pct_ctx* c, float* dst, int64_t n_voxels) {
     if (!c) return PCT_EINVAL;
     if (!dst || n_voxels != c->n_voxels) return fail(c, PCT_EINVAL, "pct_get_image: dst NULL or n_voxels != nx*ny*nz");
+    if (int rc = wait_upload(c, -1)) return rc;
     CUDA_TRY(c, cudaMemcpyAsync(dst, c->x, sizeof(float) * c->n_voxels, cudaMemcpyDefault, c->stream));
     CUDA_TRY(c, cudaStreamSynchronize(c->stream));
     return PCT_OK;
@@ -363,6 +434,7 @@ extern "C" int pct_debug_rows(pct_ctx* c, int64_t first, int64_t count, int32_t 
     a.tab = c->tab;
     a.nseg = nseg; a.nnz = nnz; a.seg_idx = seg_idx;
     a.seg_len = seg_len; a.row_len = row_len; a.nodes = nodes;
+    if (int rc = wait_upload(c, first + count)) return rc;
     CUDA_TRY(c, launch_rows(a, c->stream));
     return PCT_OK;
 }
@@ -373,6 +445,7 @@ extern "C" int pct_debug_block(pct_ctx* c, int64_t first, int64_t count, float* 
     if (first < 0 || count < 1 || first + count > c->n) return fail(c, PCT_EINVAL, "pct_debug_block: range outside the histories");
     if (!delta || !cnt || !is_device_ptr(delta) || !is_device_ptr(cnt))
         return fail(c, PCT_EINVAL, "pct_debug_block: delta and cnt must be device memory");
+    if (int rc = wait_upload(c, first + count)) return rc;
     CUDA_TRY(c, cudaMemsetAsync(c->ctrl, 0, sizeof(Ctrl), c->stream));
     const DropArgs a = drop_args(c, count, first, count);
     CUDA_TRY(c, launch_drop_block(a, c->drop_grid, c->stream));
@@ -387,6 +460,7 @@ extern "C" int pct_profile_sweep(pct_ctx* c, float lambda, int64_t block_size, f
     if (!c->have_hist) return fail(c, PCT_ESTATE, "pct_profile_sweep: no histories set");
     if (!(lambda > 0.0f) || !(lambda < 2.0f)) return fail(c, PCT_EINVAL, "pct_profile_sweep: lambda must be in (0, 2)");
     if (block_size < 1 || block_size > (1LL << 24)) return fail(c, PCT_EINVAL, "pct_profile_sweep: block_size must be in [1, 2^24]");
+    if (int rc = wait_upload(c, -1)) return rc;
     const long long n_blocks = (c->n + block_size - 1) / block_size;
     const int kChunk = 256;  // blocks per batch of events
     cudaEvent_t ev[2 * kChunk + 1];

@@ -321,6 +321,51 @@ def test_host_entry_point_matches_device_entry_point(oracle_mod, pct, torch_cuda
     assert np.linalg.norm(imgs[0] - imgs[1]) <= 1e-5 * np.linalg.norm(imgs[0])
 
 
+def test_pipelined_host_upload_spans_several_chunks(pct, torch_cuda):
+    """pct_set_histories_host uploads in chunks of 2^20 .. 2^24 histories on a copy stream and the first
+    sweep starts before the upload has finished: 9.5e6 histories (five chunks, the last one ragged) from
+    pinned host arrays must give the image the device entry point gives -- for the first sweep, after
+    the host arrays are overwritten once pct_synchronize has returned, for the inspection entry point
+    on the last chunk, and for a SECOND set of the same size, which reuses the device block."""
+    import synth.cuda_gen as cuda_gen
+
+    torch = torch_cuda
+    cfg = synth.config(0)
+    n, B = 9_500_000, 20_000
+    tables = ("proj_cos", "proj_sin")
+    D2 = synth.to_pct_names(cuda_gen.generate_cuda(cfg, 2 * n))
+    sets = [{k: (v if k in tables else v[i * n:(i + 1) * n].contiguous()) for k, v in D2.items()} for i in range(2)]
+    res = []
+    for use_host in (False, True):
+        ctx = _ctx(pct, torch, cfg)
+        try:
+            for D in sets:
+                if use_host:
+                    host = {k: torch.empty(v.shape, dtype=v.dtype, pin_memory=True).copy_(v) for k, v in D.items()}
+                    torch.cuda.synchronize()
+                    pct.pct_set_histories_host(ctx, n, host)
+                else:
+                    pct.pct_set_histories(ctx, n, D)
+                pct.pct_iterate(ctx, cfg.lam, B, 1)
+                if use_host:
+                    pct.pct_synchronize(ctx)
+                    host["wepl"].fill_(1.0e9)  # the library may not read the host arrays any more
+                pct.pct_iterate(ctx, cfg.lam, B, 1)
+                out = torch.empty(cfg.n_voxels, dtype=torch.float32, device="cuda")
+                pct.pct_get_image(ctx, out, cfg.n_voxels)
+                res.append(out.cpu().numpy())
+                nseg, nnz = _gpu_rows(pct, torch, ctx, n - 64, 64, min(cfg.nx, cfg.ny))[:2]
+                res.append(np.concatenate([nseg, nnz]))
+        finally:
+            pct.pct_destroy(ctx)
+    dev, hst = res[:4], res[4:]
+    assert np.isfinite(dev[0]).all() and np.abs(dev[0]).max() > 0.1
+    assert not np.array_equal(dev[1], dev[3])  # the two sets differ
+    for i in (0, 2):
+        assert np.linalg.norm(dev[i] - hst[i]) <= 1e-5 * np.linalg.norm(dev[i])
+        assert np.array_equal(dev[i + 1], hst[i + 1])
+
+
 def test_error_reporting(pct, torch_cuda):
     torch = torch_cuda
     cfg = synth.config(0)

@@ -39,6 +39,13 @@ struct pct_ctx {
     size_t chunks_waited = 0;  // events [0, chunks_waited) are already ordered before c->stream's tail
     long long owned_n = 0;     // histories the owned block was sized for (reused by the next upload of the same size)
     int owned_n_proj = 0;
+    // processing order of the histories inside each DROP block (k_order_blocks), built per block size
+    uint32_t* order = nullptr;
+    double l2_bytes = 0.0;      // cudaDevAttrL2CacheSize
+    int order_slabs = 4;
+    long long order_block = 0;  // block size the order was built for
+    long long order_built = 0;  // blocks [0, order_built) are ordered
+    const void* graph_order = nullptr;
     // cached CUDA graph of kGraphPairs (accumulate, update) pairs
     cudaGraphExec_t graph = nullptr;
     float graph_lambda = 0.f;
@@ -120,8 +127,55 @@ static int wait_upload(pct_ctx* c, long long upto) {
     return PCT_OK;
 }
 
+#ifndef PCT_ORDER_BLOCKS
+#define PCT_ORDER_BLOCKS 1  // 0: never, 1: when image + accumulator exceed 85 % of the L2, 2: always
+#endif
+
+// The order buffer for this block size (4 B per history); without memory for it the blocks run in the
+// caller's order.  Slabs: image + accumulator (12 B per voxel) of one slab take a quarter of the L2, at
+// least 4 (measured at 256 x 256 x 160, 126 MB: 440 -> 317 us per 2e5-history block with 4 slabs, 318
+// with 8, 323 with 16; at 256 x 256 x 128, 101 MB: 169.3 -> 166.9 us, k_update 23.2 -> 24.3 us).
+static void prepare_order(pct_ctx* c, long long block_size) {
+    const double l2 = c->l2_bytes > 0.0 ? c->l2_bytes : 128.0e6;
+    // ordering pays when image + accumulator do not fit the L2; for a grid that fits it is a wash (256 x 256 x
+    // 128, 101 MB: sweep 906 -> 910 ms, and every upload would pay the sort), so such grids keep the caller's
+    // order and its coalesced history loads
+    int mode = PCT_ORDER_BLOCKS;
+    if (const char* env = getenv("PCT_ORDER"))  // tuning / test override: 0 never, 1 by footprint, 2 always
+        if (env[0] >= '0' && env[0] <= '2' && env[1] == 0) mode = env[0] - '0';
+    const bool wanted = mode == 2 || (mode == 1 && 12.0 * (double)c->n_voxels > 0.85 * l2);
+    if (!wanted || block_size < 1024) {  // (small blocks: nothing to gain)
+        if (c->order) cudaFree(c->order);
+        c->order = nullptr;
+        c->order_block = 0;
+        return;
+    }
+    const double per_slab = 0.25 * l2;
+    const double want = ceil(12.0 * (double)c->n_voxels / per_slab);
+    c->order_slabs = want < 4.0 ? 4 : (want > 64.0 ? 64 : (int)want);
+    if (c->order && c->order_block == block_size) return;
+    if (!c->order && cudaMalloc(&c->order, sizeof(uint32_t) * (size_t)c->n) != cudaSuccess) {
+        (void)cudaGetLastError();
+        c->order = nullptr;
+    }
+    c->order_block = block_size;
+    c->order_built = 0;
+}
+
+// Order DROP blocks [order_built, upto) (their histories must be on the device or on their way in c->stream's order).
+static int build_order(pct_ctx* c, long long block_size, long long upto) {
+    if (!c->order || upto <= c->order_built) return PCT_OK;
+    CUDA_TRY(c, launch_order_blocks(c->H, c->g, c->n, block_size, c->order_built, upto - c->order_built, c->order_slabs, c->order, c->stream));
+    c->order_built = upto;
+    return PCT_OK;
+}
+
 static void release_histories(pct_ctx* c) {
     drop_graph(c);
+    if (c->order) cudaFree(c->order);
+    c->order = nullptr;
+    c->order_block = 0;
+    c->order_built = 0;
     if (!c->chunk_ev.empty()) {
         if (c->copy_stream) cudaStreamSynchronize(c->copy_stream);
         for (cudaEvent_t e : c->chunk_ev) cudaEventDestroy(e);
@@ -172,6 +226,9 @@ extern "C" int pct_create(pct_ctx** out, int nx, int ny, int nz, float h, float 
     int rc = PCT_OK;
     auto body = [&]() -> int {
         CUDA_TRY(nullptr, cudaGetDevice(&c->device));
+        int l2 = 0;
+        CUDA_TRY(nullptr, cudaDeviceGetAttribute(&l2, cudaDevAttrL2CacheSize, c->device));
+        c->l2_bytes = (double)l2;
         CUDA_TRY(nullptr, cudaMalloc(&c->x, sizeof(float) * c->n_voxels));
         CUDA_TRY(nullptr, cudaMalloc(&c->acc, sizeof(float2) * c->n_voxels));
         CUDA_TRY(nullptr, cudaMalloc(&c->tab, sizeof(float4) * (nmin + 1)));
@@ -268,6 +325,7 @@ extern "C" int pct_set_histories_host(pct_ctx* c, int64_t n, const pct_histories
         c->chunk_ev.clear();
         c->chunk_end.clear();
         c->chunks_waited = 0;
+        c->order_built = 0;  // same buffer, new histories: the blocks are ordered again as they arrive
         cudaEvent_t tail = nullptr;
         CUDA_TRY(c, cudaEventCreateWithFlags(&tail, cudaEventDisableTiming));
         cudaError_t e = cudaEventRecord(tail, c->stream);
@@ -321,6 +379,7 @@ static DropArgs drop_args(pct_ctx* c, long long block_size, long long first, lon
     a.acc = c->acc;
     a.tab = c->tab;
     a.ctrl = c->ctrl;
+    a.order = first < 0 ? c->order : nullptr;
     return a;
 }
 
@@ -340,11 +399,16 @@ extern "C" int pct_iterate(pct_ctx* c, float lambda, int64_t block_size, int n_i
     const long long n_blocks = (c->n + block_size - 1) / block_size;
     const long long pairs = n_blocks * (long long)n_iter;
     CUDA_TRY(c, cudaMemsetAsync(c->ctrl, 0, sizeof(Ctrl), c->stream));
+    prepare_order(c, block_size);
+    if (c->chunks_waited == c->chunk_ev.size()) {  // every history is on the device: order all blocks in one launch
+        int rc = build_order(c, block_size, n_blocks);
+        if (rc) return rc;
+    }
     const DropArgs a = drop_args(c, block_size, -1, 0);
     long long done = 0;
     if (pairs >= 2 * kGraphPairs) {
         const bool reuse = c->graph && c->graph_lambda == lambda && c->graph_block == block_size && c->graph_n == c->n &&
-                           c->graph_hist_key == (const void*)c->H.t_in;
+                           c->graph_hist_key == (const void*)c->H.t_in && c->graph_order == (const void*)c->order;
         if (!reuse) {
             drop_graph(c);
             cudaStream_t cap = nullptr;
@@ -365,16 +429,19 @@ extern "C" int pct_iterate(pct_ctx* c, float lambda, int64_t block_size, int n_i
             c->graph_block = block_size;
             c->graph_n = c->n;
             c->graph_hist_key = (const void*)c->H.t_in;
+            c->graph_order = (const void*)c->order;
         }
         for (; done + kGraphPairs <= pairs; done += kGraphPairs) {
             // blocks done .. done+63 of the first sweep need the histories below (done + 64) * block_size
             int rc = wait_upload(c, done + kGraphPairs <= n_blocks ? (done + kGraphPairs) * block_size : -1);
+            if (rc == PCT_OK) rc = build_order(c, block_size, done + kGraphPairs <= n_blocks ? done + kGraphPairs : n_blocks);
             if (rc) return rc;
             CUDA_TRY(c, cudaGraphLaunch(c->graph, c->stream));
         }
     }
     for (; done < pairs; ++done) {
         int rc = wait_upload(c, done < n_blocks ? (done + 1) * block_size : -1);
+        if (rc == PCT_OK) rc = build_order(c, block_size, done < n_blocks ? done + 1 : n_blocks);
         if (rc == PCT_OK) rc = enqueue_pair(c, a, lambda, n_blocks, c->stream);
         if (rc) return rc;
     }
@@ -470,6 +537,8 @@ extern "C" int pct_profile_sweep(pct_ctx* c, float lambda, int64_t block_size, f
     auto body = [&]() -> int {
         for (; made < 2 * kChunk + 1; ++made) CUDA_TRY(c, cudaEventCreate(&ev[made]));
         CUDA_TRY(c, cudaMemsetAsync(c->ctrl, 0, sizeof(Ctrl), c->stream));
+        prepare_order(c, block_size);
+        if (int rc2 = build_order(c, block_size, n_blocks)) return rc2;
         const DropArgs a = drop_args(c, block_size, -1, 0);
         for (long long b0 = 0; b0 < n_blocks; b0 += kChunk) {
             const int nb = (int)(n_blocks - b0 < kChunk ? n_blocks - b0 : kChunk);

@@ -36,6 +36,8 @@ struct DropArgs {
     float2* acc;           // (Delta_j, c_j) interleaved
     const float4* tab;     // Sigma1^-1 table, nmin+1 entries
     Ctrl* ctrl;
+    const uint32_t* order; // block mode: order[b*block_size + r] = offset inside DROP block b of the r-th
+                           // history to process (k_order_blocks); nullptr: the caller's order
 };
 
 struct RowsArgs {
@@ -56,5 +58,7 @@ cudaError_t launch_update(float* x, float2* acc, long long n_voxels, float lambd
                           long long n_blocks, cudaStream_t stream);
 cudaError_t launch_split_acc(float2* acc, float* delta, float* cnt, long long n_voxels, cudaStream_t stream);
 cudaError_t launch_rows(const RowsArgs& a, cudaStream_t stream);
+cudaError_t launch_order_blocks(const HistPtrs& H, const Geom& g, long long n, long long block_size, long long first_block,
+                                long long n_blocks, int n_slabs, uint32_t* order, cudaStream_t stream);
 
 }  // namespace pct

@@ -408,6 +408,7 @@ struct Queue {
     long long hist0[kPhases];           // first history of the phase (relative to `first`)
     unsigned long long n_static;        // tickets [0, n_static) are owned by warps, not drawn
     unsigned long long n_items;
+    bool interleave;                    // static items strided by n_static (ordered blocks)
 };
 
 __device__ __forceinline__ Queue make_queue(long long first, long long count, long long n_warps) {
@@ -443,12 +444,23 @@ __device__ __forceinline__ Queue make_queue(long long first, long long count, lo
     return q;
 }
 
-__device__ __forceinline__ void queue_item(const Queue& q, unsigned long long w, long long& i0, int& cnt) {
+// Item w: histories rel0, rel0 + stride, ... (cnt of them), positions in the block's processing order.
+// With the histories of a block ordered by depth slab (k_order_blocks) the static items are INTERLEAVED
+// (item w takes positions w, w + n_static, w + 2 n_static, ...), so that all warps move through the order
+// together and the grid works on one slab of the image at a time.  All other items are contiguous.
+__device__ __forceinline__ void queue_item(const Queue& q, unsigned long long w, long long& rel0, int& cnt, long long& stride) {
     int p = 0;
 #pragma unroll
     for (int t = 1; t < kPhases; ++t) p = w >= q.item0[t] ? t : p;
+    if (p == 0 && q.interleave) {
+        rel0 = (long long)w;
+        stride = (long long)q.n_static;
+        cnt = q.size[0];
+        return;
+    }
     const long long rel = q.hist0[p] + (long long)(w - q.item0[p]) * q.size[p];
-    i0 = q.first + rel;
+    rel0 = rel;
+    stride = 1;
     const long long left = q.count - rel;
     cnt = left < q.size[p] ? (int)left : q.size[p];
 }
@@ -469,6 +481,7 @@ __global__ void __launch_bounds__(kThreads, kCtasPerSm) k_drop_block(const DropA
             count = a.n - first < a.block_size ? a.n - first : a.block_size;
         }
         q = make_queue(first, count, (long long)gridDim.x * kWarpsPerCta);
+        q.interleave = a.first < 0 && a.order != nullptr;
     }
     stage_table(s_tab, a.tab, g.nmin);  // (ends with __syncthreads: q is visible)
     unsigned long long rows = 0, nnz_total = 0, segs = 0;
@@ -482,11 +495,13 @@ __global__ void __launch_bounds__(kThreads, kCtasPerSm) k_drop_block(const DropA
             w = __shfl_sync(0xffffffffu, w, 0);
         }
         if (w >= q.n_items) break;
-        long long i0;
+        long long rel0, stride;
         int cnt;
-        queue_item(q, w, i0, cnt);
+        queue_item(q, w, rel0, cnt, stride);
         if (lane < cnt) {
-            const Hist hh = load_history(a.H, i0 + lane);
+            long long r = rel0 + lane * stride;  // position in the processing order of the block
+            if (q.interleave) r = (long long)__ldg(a.order + q.first + r);  // ordered block (k_order_blocks)
+            const Hist hh = load_history(a.H, q.first + r);
             setup_history(g, hh, s_state[lane]);
         }
         __syncwarp();
@@ -736,6 +751,66 @@ cudaError_t launch_rows(const RowsArgs& a, cudaStream_t stream) {
     e = cudaFuncSetAttribute(k_rows, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (e == cudaSuccess) k_rows<<<(int)blocks, kThreads, smem, stream>>>(a);
     if (e != cudaSuccess) return e;
+    return cudaGetLastError();
+}
+
+// ---- processing order of the histories inside a DROP block -------------------------------------
+// The block update is a sum over the rows of the block (R12), so the library may take them in any
+// order (R14: never across blocks).  A path stays within a slice or two of the image (mrad slopes),
+// so histories taken DEPTH SLAB by depth slab touch 1/n_slabs of image and accumulator at a time:
+// the gather and the reductions hit the L2 even when image + accumulator (126 MB at 256 x 256 x 160)
+// exceed it.  One counting sort per block on the slab of the straight entry ray at u = 0.  An ordering
+// only: any key gives the same sums.  (A second key, longest histories first inside a slab so that the
+// launch ends on short ones, was measured: no gain.)
+constexpr int kOrderBins = 64;  // at most that many slabs
+
+__device__ __forceinline__ int order_key(const HistPtrs& H, const Geom& g, int n_slabs, long long i) {
+    const float vc = __ldg(H.v_in + i) - __ldg(H.dv_in + i) * g.u_in;  // straight entry ray at u = 0
+    float fs = (vc + g.zmax) / (2.0f * g.zmax) * (float)n_slabs;
+    fs = fs >= 0.0f ? fs : 0.0f;  // (NaN -> 0)
+    return fs < (float)n_slabs ? (int)fs : n_slabs - 1;
+}
+
+__global__ void __launch_bounds__(512) k_order_blocks(const HistPtrs H, const Geom g, long long n, long long block_size,
+                                                      long long first_block, long long n_blocks, int n_slabs, uint32_t* __restrict__ order) {
+    __shared__ unsigned bins[kOrderBins];
+    for (long long b = first_block + blockIdx.x; b < first_block + n_blocks; b += gridDim.x) {
+        const long long first = b * block_size;
+        const long long count = n - first < block_size ? n - first : block_size;
+        for (int k = threadIdx.x; k < kOrderBins; k += blockDim.x) bins[k] = 0u;
+        __syncthreads();
+        for (long long r = threadIdx.x; r < count; r += blockDim.x) atomicAdd(&bins[order_key(H, g, n_slabs, first + r)], 1u);
+        __syncthreads();
+        if (threadIdx.x < 32) {  // exclusive scan of the bin counts by one warp
+            unsigned carry = 0u;
+            for (int k0 = 0; k0 < kOrderBins; k0 += 32) {
+                const int k = k0 + threadIdx.x;
+                const unsigned c = k < kOrderBins ? bins[k] : 0u;
+                unsigned incl = c;
+#pragma unroll
+                for (int o = 1; o < 32; o <<= 1) {
+                    const unsigned up = __shfl_up_sync(0xffffffffu, incl, o);
+                    if ((int)threadIdx.x >= o) incl += up;
+                }
+                if (k < kOrderBins) bins[k] = carry + incl - c;
+                carry += __shfl_sync(0xffffffffu, incl, 31);
+            }
+        }
+        __syncthreads();
+        for (long long r = threadIdx.x; r < count; r += blockDim.x) {
+            const unsigned pos = atomicAdd(&bins[order_key(H, g, n_slabs, first + r)], 1u);
+            order[first + pos] = (uint32_t)r;
+        }
+        __syncthreads();
+    }
+}
+
+cudaError_t launch_order_blocks(const HistPtrs& H, const Geom& g, long long n, long long block_size, long long first_block,
+                                long long n_blocks, int n_slabs, uint32_t* order, cudaStream_t stream) {
+    if (n_blocks < 1) return cudaSuccess;
+    n_slabs = n_slabs < 1 ? 1 : (n_slabs > kOrderBins ? kOrderBins : n_slabs);
+    const long long grid = n_blocks < 148 * 4 ? n_blocks : 148 * 4;
+    k_order_blocks<<<(int)grid, 512, 0, stream>>>(H, g, n, block_size, first_block, n_blocks, n_slabs, order);
     return cudaGetLastError();
 }
 

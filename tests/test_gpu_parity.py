@@ -321,13 +321,18 @@ def test_host_entry_point_matches_device_entry_point(oracle_mod, pct, torch_cuda
     assert np.linalg.norm(imgs[0] - imgs[1]) <= 1e-5 * np.linalg.norm(imgs[0])
 
 
-def test_pipelined_host_upload_spans_several_chunks(pct, torch_cuda):
+@pytest.mark.parametrize("order", ["1", "2"])
+def test_pipelined_host_upload_spans_several_chunks(pct, torch_cuda, monkeypatch, order):
     """pct_set_histories_host uploads in chunks of 2^20 .. 2^24 histories on a copy stream and the first
     sweep starts before the upload has finished: 9.5e6 histories (five chunks, the last one ragged) from
     pinned host arrays must give the image the device entry point gives -- for the first sweep, after
     the host arrays are overwritten once pct_synchronize has returned, for the inspection entry point
-    on the last chunk, and for a SECOND set of the same size, which reuses the device block."""
+    on the last chunk, and for a SECOND set of the same size, which reuses the device block.  order = "2"
+    forces the depth-slab ordering of the DROP blocks (by default only grids larger than the L2 get it), whose
+    sort then runs batch by batch behind the upload."""
     import synth.cuda_gen as cuda_gen
+
+    monkeypatch.setenv("PCT_ORDER", order)
 
     torch = torch_cuda
     cfg = synth.config(0)

@@ -12,6 +12,7 @@ from .binding import (  # noqa: F401
     Histories,
     block_accumulate,
     build,
+    carp_iterate,
     drop_iterate,
     lib,
     mlp_chi2_f64,

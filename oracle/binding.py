@@ -136,6 +136,8 @@ def lib():
                                            C.c_int64, dp, dp, ip, C.POINTER(C.c_int64), C.c_int]
         L.orc_drop_iterate.argtypes = [C.POINTER(_Geom), C.POINTER(_Histories), C.c_int64, C.c_double,
                                        C.c_int64, C.c_int, dp, C.POINTER(C.c_int64), C.c_int]
+        L.orc_carp_iterate.argtypes = [C.POINTER(_Geom), C.POINTER(_Histories), C.c_int64, C.c_double,
+                                       C.c_int64, C.c_int, C.c_int, dp, C.c_int]
         L.orc_num_threads.restype = C.c_int
         _lib = L
     return _lib
@@ -253,6 +255,19 @@ def drop_iterate(geom, hists, lam, block_size, n_iter, x, n=None, nthreads=0):
     if rc:
         raise RuntimeError("orc_drop_iterate failed: %d" % rc)
     return x, tuple(stats)
+
+
+def carp_iterate(geom, hists, lam, block_size, n_iter, n_strings, x, n=None, nthreads=0):
+    """n_iter CARP iterations in place on x (float64[M]): n_strings strings from a common
+    x0, each one DROP sweep over its own histories, then the mean of the string solutions."""
+    x = np.ascontiguousarray(x, dtype=np.float64)
+    assert x.shape == (geom.n_voxels,)
+    g, hs = geom.c(), hists.c()
+    rc = lib().orc_carp_iterate(C.byref(g), C.byref(hs), int(hists.n if n is None else n), float(lam),
+                                int(block_size), int(n_iter), int(n_strings), _dp(x), int(nthreads))
+    if rc:
+        raise RuntimeError("orc_carp_iterate failed: %d" % rc)
+    return x
 
 
 def num_threads():

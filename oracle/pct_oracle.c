@@ -654,6 +654,48 @@ int orc_drop_iterate(const orc_geom *g, const orc_histories *H, int64_t n, doubl
     return 0;
 }
 
+/* CARP (section 2.2 and Fig. 2; readings R27-R29), n_iter iterations, x (M doubles)
+ * in/out.  "The data are ... distributed among a user-determined number of blocks (strings in CARP
+ * terminology) ... we proceed to get a new estimate x_n for each data subset n using the same initial guess
+ * x_0.  A new solution is then computed from the average of the different string solutions ... if a new
+ * iteration is desired, the initial solution for all the subsets will be this average."
+ *   strings   string p = histories [floor(p n / P), floor((p+1) n / P)) of the caller's order (R27)
+ *   estimate  one sweep of the block iteration of section 2.1 over the string's histories, in blocks of
+ *             block_size counted from the string's first history, starting from the common x_0 (R28)
+ *   average   the arithmetic mean of the P string solutions, voxel by voxel (R29)                         */
+int orc_carp_iterate(const orc_geom *g, const orc_histories *H, int64_t n, double lambda, int64_t block_size,
+                     int n_iter, int n_strings, double *x, int nthreads) {
+    const int64_t M = (int64_t)g->nx * g->ny * g->nz;
+    if (n <= 0 || block_size <= 0 || n_iter < 0 || n_strings < 1 || n_strings > n) return -1;
+    double *delta = (double *)malloc(sizeof(double) * (size_t)M);
+    double *xs = (double *)malloc(sizeof(double) * (size_t)M);
+    double *sum = (double *)malloc(sizeof(double) * (size_t)M);
+    int32_t *cnt = (int32_t *)malloc(sizeof(int32_t) * (size_t)M);
+    int rc = (!delta || !xs || !sum || !cnt) ? -2 : 0;
+    for (int it = 0; it < n_iter && rc == 0; ++it) {
+        for (int64_t j = 0; j < M; ++j) sum[j] = 0.0;
+        for (int p = 0; p < n_strings && rc == 0; ++p) {
+            const int64_t lo = (int64_t)(((__int128)p * n) / n_strings), hi = (int64_t)(((__int128)(p + 1) * n) / n_strings);
+            for (int64_t j = 0; j < M; ++j) xs[j] = x[j];
+            for (int64_t first = lo; first < hi && rc == 0; first += block_size) {
+                const int64_t count = hi - first < block_size ? hi - first : block_size;
+                int64_t st[3];
+                rc = orc_block_accumulate(g, H, first, count, xs, delta, cnt, st, nthreads);
+                if (rc) break;
+                for (int64_t j = 0; j < M; ++j) {
+                    const int32_t c = cnt[j] > 1 ? cnt[j] : 1;
+                    xs[j] += lambda * delta[j] / (double)c;
+                }
+            }
+            for (int64_t j = 0; j < M; ++j) sum[j] += xs[j];
+        }
+        if (rc == 0)
+            for (int64_t j = 0; j < M; ++j) x[j] = sum[j] / (double)n_strings;
+    }
+    free(delta); free(xs); free(sum); free(cnt);
+    return rc;
+}
+
 int orc_num_threads(void) {
 #ifdef _OPENMP
     return omp_get_max_threads();

@@ -16,6 +16,7 @@ from .binding import (  # noqa: F401
     pct_get_image,
     pct_get_stats,
     pct_iterate,
+    pct_iterate_carp,
     pct_profile_sweep,
     pct_set_histories,
     pct_set_histories_host,

@@ -46,6 +46,7 @@ def lib():
         L.pct_set_histories.argtypes = [vp, i64, C.POINTER(pct_histories)]
         L.pct_set_histories_host.argtypes = [vp, i64, C.POINTER(pct_histories)]
         L.pct_iterate.argtypes = [vp, C.c_float, i64, C.c_int]
+        L.pct_iterate_carp.argtypes = [vp, C.c_float, i64, C.c_int, C.c_int]
         L.pct_get_image.argtypes = [vp, vp, i64]
         L.pct_set_image.argtypes = [vp, vp, i64]
         L.pct_synchronize.argtypes = [vp]
@@ -62,7 +63,7 @@ def lib():
     return _lib
 
 
-EXPORTS = ("pct_create", "pct_set_histories", "pct_set_histories_host", "pct_iterate", "pct_get_image",
+EXPORTS = ("pct_create", "pct_set_histories", "pct_set_histories_host", "pct_iterate", "pct_iterate_carp", "pct_get_image",
            "pct_set_image", "pct_synchronize", "pct_get_stats", "pct_destroy", "pct_last_error", "pct_version",
            "pct_debug_rows", "pct_debug_block", "pct_profile_sweep")
 
@@ -120,6 +121,10 @@ def pct_set_histories_host(ctx, n, arrays):
 
 def pct_iterate(ctx, lam, block_size, n_iter):
     _check(ctx, lib().pct_iterate(ctx, float(lam), int(block_size), int(n_iter)))
+
+
+def pct_iterate_carp(ctx, lam, block_size, n_iter, n_strings):
+    _check(ctx, lib().pct_iterate_carp(ctx, float(lam), int(block_size), int(n_iter), int(n_strings)))
 
 
 def pct_get_image(ctx, dst, n_voxels):

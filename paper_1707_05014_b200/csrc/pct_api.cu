@@ -46,6 +46,14 @@ struct pct_ctx {
     long long order_block = 0;  // block size the order was built for
     long long order_built = 0;  // blocks [0, order_built) are ordered
     const void* graph_order = nullptr;
+    // CARP (pct_iterate_carp): one image, accumulator, control block and stream per string
+    int carp_p = 0;
+    float* carp_x = nullptr;
+    float2* carp_acc = nullptr;
+    Ctrl* carp_ctrl = nullptr;
+    std::vector<cudaStream_t> carp_stream;
+    std::vector<cudaEvent_t> carp_done;
+    cudaEvent_t carp_fork = nullptr;
     // cached CUDA graph of kGraphPairs (accumulate, update) pairs
     cudaGraphExec_t graph = nullptr;
     float graph_lambda = 0.f;
@@ -258,9 +266,29 @@ extern "C" int pct_create(pct_ctx** out, int nx, int ny, int nz, float h, float 
     return PCT_OK;
 }
 
+static void release_carp(pct_ctx* c) {
+    for (cudaStream_t s : c->carp_stream) {
+        cudaStreamSynchronize(s);
+        cudaStreamDestroy(s);
+    }
+    for (cudaEvent_t e : c->carp_done) cudaEventDestroy(e);
+    c->carp_stream.clear();
+    c->carp_done.clear();
+    if (c->carp_fork) cudaEventDestroy(c->carp_fork);
+    c->carp_fork = nullptr;
+    if (c->carp_x) cudaFree(c->carp_x);
+    if (c->carp_acc) cudaFree(c->carp_acc);
+    if (c->carp_ctrl) cudaFree(c->carp_ctrl);
+    c->carp_x = nullptr;
+    c->carp_acc = nullptr;
+    c->carp_ctrl = nullptr;
+    c->carp_p = 0;
+}
+
 extern "C" void pct_destroy(pct_ctx* c) {
     if (!c) return;
     cudaStreamSynchronize(c->stream);
+    release_carp(c);
     release_histories(c);
     if (c->copy_stream) cudaStreamDestroy(c->copy_stream);
     if (c->x) cudaFree(c->x);
@@ -444,6 +472,69 @@ extern "C" int pct_iterate(pct_ctx* c, float lambda, int64_t block_size, int n_i
         if (rc == PCT_OK) rc = build_order(c, block_size, done < n_blocks ? done + 1 : n_blocks);
         if (rc == PCT_OK) rc = enqueue_pair(c, a, lambda, n_blocks, c->stream);
         if (rc) return rc;
+    }
+    return PCT_OK;
+}
+
+// CARP (Fig. 2; R27-R29).  Every string runs its DROP sweep on a stream of its
+// own, with its own image copy, accumulator and control block, so the strings' kernels overlap: the tail of
+// one string's block launch and its update kernel are filled by the other strings' blocks.
+extern "C" int pct_iterate_carp(pct_ctx* c, float lambda, int64_t block_size, int n_iter, int n_strings) {
+    if (!c) return PCT_EINVAL;
+    if (!c->have_hist) return fail(c, PCT_ESTATE, "pct_iterate_carp: no histories set");
+    if (!(lambda > 0.0f) || !(lambda < 2.0f)) return fail(c, PCT_EINVAL, "pct_iterate_carp: lambda must be in (0, 2)");
+    if (block_size < 1 || block_size > (1LL << 24)) return fail(c, PCT_EINVAL, "pct_iterate_carp: block_size must be in [1, 2^24]");
+    if (n_iter < 0) return fail(c, PCT_EINVAL, "pct_iterate_carp: n_iter must be >= 0");
+    if (n_strings < 1 || n_strings > 64 || (long long)n_strings > c->n)
+        return fail(c, PCT_EINVAL, "pct_iterate_carp: n_strings must be in [1, min(64, n)]");
+    if (n_iter == 0) return PCT_OK;
+    if (int rc = wait_upload(c, -1)) return rc;
+    const int P = n_strings;
+    const long long M = c->n_voxels;
+    if (c->carp_p != P) {
+        release_carp(c);
+        CUDA_TRY(c, cudaMalloc(&c->carp_x, sizeof(float) * (size_t)M * P));
+        CUDA_TRY(c, cudaMalloc(&c->carp_acc, sizeof(float2) * (size_t)M * P));
+        CUDA_TRY(c, cudaMalloc(&c->carp_ctrl, sizeof(Ctrl) * P));
+        CUDA_TRY(c, cudaMemsetAsync(c->carp_acc, 0, sizeof(float2) * (size_t)M * P, c->stream));
+        CUDA_TRY(c, cudaEventCreateWithFlags(&c->carp_fork, cudaEventDisableTiming));
+        for (int p = 0; p < P; ++p) {
+            cudaStream_t s = nullptr;
+            cudaEvent_t e = nullptr;
+            CUDA_TRY(c, cudaStreamCreateWithFlags(&s, cudaStreamNonBlocking));
+            c->carp_stream.push_back(s);
+            CUDA_TRY(c, cudaEventCreateWithFlags(&e, cudaEventDisableTiming));
+            c->carp_done.push_back(e);
+        }
+        c->carp_p = P;
+    }
+    for (int it = 0; it < n_iter; ++it) {
+        CUDA_TRY(c, cudaEventRecord(c->carp_fork, c->stream));  // x (and, the first time, the zeroed accumulators) are ready
+        for (int p = 0; p < P; ++p) {
+            cudaStream_t s = c->carp_stream[p];
+            const long long lo = (long long)(((__int128)p * c->n) / P), hi = (long long)(((__int128)(p + 1) * c->n) / P);
+            float* xs = c->carp_x + (size_t)p * M;
+            CUDA_TRY(c, cudaStreamWaitEvent(s, c->carp_fork, 0));
+            CUDA_TRY(c, cudaMemcpyAsync(xs, c->x, sizeof(float) * M, cudaMemcpyDeviceToDevice, s));  // the common x0
+            CUDA_TRY(c, cudaMemsetAsync(c->carp_ctrl + p, 0, sizeof(Ctrl), s));
+            DropArgs a = drop_args(c, block_size, -1, 0);
+            a.H.t_in += lo; a.H.v_in += lo; a.H.t_out += lo; a.H.v_out += lo;
+            a.H.dt_in += lo; a.H.dv_in += lo; a.H.dt_out += lo; a.H.dv_out += lo;
+            a.H.wepl += lo; a.H.proj += lo;
+            a.n = hi - lo;
+            a.x = xs;
+            a.acc = c->carp_acc + (size_t)p * M;
+            a.ctrl = c->carp_ctrl + p;
+            a.order = nullptr;
+            const long long n_blocks = (a.n + block_size - 1) / block_size;
+            for (long long b = 0; b < n_blocks; ++b) {
+                CUDA_TRY(c, launch_drop_block(a, c->drop_grid, s));
+                CUDA_TRY(c, launch_update(xs, a.acc, M, lambda, a.ctrl, n_blocks, s));
+            }
+            CUDA_TRY(c, cudaEventRecord(c->carp_done[p], s));
+            CUDA_TRY(c, cudaStreamWaitEvent(c->stream, c->carp_done[p], 0));
+        }
+        CUDA_TRY(c, launch_mean(c->x, c->carp_x, P, M, c->stream));
     }
     return PCT_OK;
 }

@@ -58,6 +58,7 @@ cudaError_t launch_update(float* x, float2* acc, long long n_voxels, float lambd
                           long long n_blocks, cudaStream_t stream);
 cudaError_t launch_split_acc(float2* acc, float* delta, float* cnt, long long n_voxels, cudaStream_t stream);
 cudaError_t launch_rows(const RowsArgs& a, cudaStream_t stream);
+cudaError_t launch_mean(float* x, const float* xs, int n_strings, long long n_voxels, cudaStream_t stream);
 cudaError_t launch_order_blocks(const HistPtrs& H, const Geom& g, long long n, long long block_size, long long first_block,
                                 long long n_blocks, int n_slabs, uint32_t* order, cudaStream_t stream);
 

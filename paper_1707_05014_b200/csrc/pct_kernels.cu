@@ -814,4 +814,24 @@ cudaError_t launch_order_blocks(const HistPtrs& H, const Geom& g, long long n, l
     return cudaGetLastError();
 }
 
+// CARP (R29): the new solution is the arithmetic mean of the P string solutions, voxel by
+// voxel; summed in the order of the strings (deterministic).  xs = P images of n voxels, back to back.
+__global__ void __launch_bounds__(256) k_mean(float* __restrict__ x, const float* __restrict__ xs, int n_strings, long long n) {
+    const long long stride = (long long)gridDim.x * blockDim.x;
+    const float fp = (float)n_strings;
+    for (long long j = (long long)blockIdx.x * blockDim.x + threadIdx.x; j < n; j += stride) {
+        float s = 0.0f;
+        for (int p = 0; p < n_strings; ++p) s += xs[(long long)p * n + j];
+        x[j] = __fdiv_rn(s, fp);
+    }
+}
+
+cudaError_t launch_mean(float* x, const float* xs, int n_strings, long long n, cudaStream_t stream) {
+    long long blocks = (n + 255) / 256;
+    if (blocks > 148 * 8) blocks = 148 * 8;
+    if (blocks < 1) blocks = 1;
+    k_mean<<<(int)blocks, 256, 0, stream>>>(x, xs, n_strings, n);
+    return cudaGetLastError();
+}
+
 }  // namespace pct

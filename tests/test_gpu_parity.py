@@ -241,6 +241,77 @@ def test_config1_sample(oracle_mod, pct, torch_cuda):
     _run_parity(oracle_mod, pct, torch_cuda, cfg, H, cfg.lam, cfg.block_size, 2)
 
 
+def _carp_parity(oracle, pct, torch, cfg, H, lam, block, n_iter, n_strings, x0=None):
+    """CARP run (R27-R29), image compared with the oracle after every iteration."""
+    geom = oracle_geom(oracle, cfg)
+    hs = oracle.Histories(H)
+    D = to_device(H)
+    M = cfg.n_voxels
+    x_ref = np.zeros(M) if x0 is None else x0.astype(np.float32).astype(np.float64)
+    ctx = _ctx(pct, torch, cfg)
+    out = torch.zeros(M, dtype=torch.float32, device="cuda")
+    try:
+        pct.pct_set_histories(ctx, hs.n, D)
+        if x0 is not None:
+            pct.pct_set_image(ctx, x0.astype(np.float32), M)
+        for it in range(n_iter):
+            pct.pct_iterate_carp(ctx, lam, block, 1, n_strings)
+            pct.pct_get_image(ctx, out, M)
+            x_ref = oracle.carp_iterate(geom, hs, lam, block, 1, n_strings, x_ref)
+            x = out.cpu().numpy().astype(np.float64)
+            rel = np.linalg.norm(x - x_ref) / np.linalg.norm(x_ref)
+            assert rel <= REL_L2_PER_ITER, "iteration %d: rel L2 %.3g" % (it, rel)
+        assert np.abs(x - x_ref).max() <= ABS_FINAL
+    finally:
+        pct.pct_destroy(ctx)
+    return x, x_ref
+
+
+@pytest.mark.parametrize("n_strings", [1, 4, 7])
+def test_carp_config0(oracle_mod, pct, torch_cuda, n_strings):
+    """configs[0] data and parameters, CARP with 1 / 4 / 7 strings (ragged strings and last blocks), 3 iterations."""
+    cfg = synth.config(0)
+    H = synth.generate_numpy(cfg, 60_011)
+    x, x_ref = _carp_parity(oracle_mod, pct, torch_cuda, cfg, H, 0.5, cfg.block_size, 3, n_strings)
+    assert np.linalg.norm(x_ref) > 1.0
+
+
+def test_carp_config1_sample_from_an_image(oracle_mod, pct, torch_cuda):
+    """configs[1] geometry and block size, 3 strings of 1e5 histories, two iterations from a non-trivial image."""
+    cfg = synth.config(1)
+    H = synth.generate_numpy(cfg, 300_000)
+    _carp_parity(oracle_mod, pct, torch_cuda, cfg, H, cfg.lam, cfg.block_size, 2, 3, x0=synth.rsp_volume(cfg) * 0.8)
+
+
+def test_carp_one_string_is_drop_and_arguments(pct, torch_cuda):
+    torch = torch_cuda
+    cfg = synth.config(0)
+    H = synth.generate_numpy(cfg, 20_000)
+    D = to_device(H)
+    imgs = []
+    for carp in (False, True):
+        ctx = _ctx(pct, torch, cfg)
+        try:
+            if carp:
+                with pytest.raises(pct.PctError):
+                    pct.pct_iterate_carp(ctx, 0.5, 1000, 1, 2)  # no histories yet
+            pct.pct_set_histories(ctx, 20_000, D)
+            if carp:
+                for bad in (0, 65, -1):
+                    with pytest.raises(pct.PctError):
+                        pct.pct_iterate_carp(ctx, 0.5, 1000, 1, bad)
+                pct.pct_iterate_carp(ctx, 0.5, 1000, 2, 1)
+                pct.pct_iterate_carp(ctx, 0.5, 1000, 0, 3)  # n_iter = 0: nothing happens
+            else:
+                pct.pct_iterate(ctx, 0.5, 1000, 2)
+            out = torch.zeros(cfg.n_voxels, dtype=torch.float32, device="cuda")
+            pct.pct_get_image(ctx, out, cfg.n_voxels)
+            imgs.append(out.cpu().numpy())
+        finally:
+            pct.pct_destroy(ctx)
+    assert np.linalg.norm(imgs[0] - imgs[1]) <= 1e-5 * np.linalg.norm(imgs[0])
+
+
 @pytest.mark.parametrize("index,n", [(3, 250_000), (4, 260_000)])
 def test_bench_launch_configuration_sample(oracle_mod, pct, torch_cuda, index, n):
     """configs[3] / configs[4] geometry with THEIR block sizes (1e5 / 2e5 histories per launch: the

@@ -57,6 +57,9 @@ def parse_args():
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu", action="store_true")
     ap.add_argument("--cpu-seconds", type=float, default=15.0, help="target CPU time of the oracle sample")
+    ap.add_argument("--carp-strings", type=int, default=0,
+                    help="P > 0: time pct_iterate_carp with P strings instead of the metric's DROP sweep (SURVEY.md 8(f) NEXT-1; "
+                         "a side measurement: one short JSON line, not the driver's contract)")
     return ap.parse_args()
 
 
@@ -370,9 +373,49 @@ def run_ours(args):
     print(json.dumps(line))
 
 
+def run_carp(args):
+    """Side measurement: one CARP iteration (P strings, each a DROP sweep over its histories, then the mean)."""
+    import torch
+
+    import paper_1707_05014_b200 as pct
+    import synth
+    import synth.cuda_gen as cuda_gen
+
+    cfg = synth.config(args.config)
+    n = cfg.n if args.histories is None else int(args.histories)
+    P = args.carp_strings
+    D = synth.to_pct_names(cuda_gen.generate_cuda(cfg, n))
+    stream = torch.cuda.Stream()
+    with torch.cuda.stream(stream):
+        ctx = pct.pct_create(cfg.nx, cfg.ny, cfg.nz, cfg.h, cfg.u_in, cfg.u_out, stream.cuda_stream)
+        try:
+            pct.pct_set_histories(ctx, n, D)
+            for _ in range(args.warmup):
+                pct.pct_iterate_carp(ctx, cfg.lam, cfg.block_size, 1, P)
+            pct.pct_synchronize(ctx)
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            with ClockSampler(0) as clk:
+                e0.record()
+                for _ in range(args.steps):
+                    pct.pct_iterate_carp(ctx, cfg.lam, cfg.block_size, 1, P)
+                e1.record()
+                torch.cuda.synchronize()
+            ms = e0.elapsed_time(e1)
+        finally:
+            pct.pct_destroy(ctx)
+    print(json.dumps({"metric": METRIC, "value": n * args.steps / (ms * 1e-3), "unit": UNIT, "n_gpus": 1, "steps": args.steps,
+                      "warmup": args.warmup, "ms_per_step": ms / args.steps, "higher_is_better": True, "dtype": "f32",
+                      "data": "synthetic", "clocks": clk.summary(),
+                      "config": {"workload": cfg.workload, "algorithm": "CARP (PAPER.md:52-56)", "strings": P, "histories": n,
+                                 "block_size": cfg.block_size, "lambda": cfg.lam,
+                                 "step": "one CARP iteration: every string one DROP sweep over its histories, then the mean"}}))
+
+
 def main():
     args = parse_args()
-    if args.impl == "reference":
+    if args.carp_strings > 0 and args.impl != "reference":
+        run_carp(args)
+    elif args.impl == "reference":
         run_reference(args)
     else:
         run_ours(args)

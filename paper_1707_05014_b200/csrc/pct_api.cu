@@ -43,6 +43,7 @@ struct pct_ctx {
     uint32_t* order = nullptr;
     double l2_bytes = 0.0;      // cudaDevAttrL2CacheSize
     int order_slabs = 4;
+    int order_strings = 0;      // 0: built for pct_iterate's blocks, P: for the blocks of P CARP strings
     long long order_block = 0;  // block size the order was built for
     long long order_built = 0;  // blocks [0, order_built) are ordered
     const void* graph_order = nullptr;
@@ -143,7 +144,10 @@ static int wait_upload(pct_ctx* c, long long upto) {
 // caller's order.  Slabs: image + accumulator (12 B per voxel) of one slab take a quarter of the L2, at
 // least 4 (measured at 256 x 256 x 160, 126 MB: 440 -> 317 us per 2e5-history block with 4 slabs, 318
 // with 8, 323 with 16; at 256 x 256 x 128, 101 MB: 169.3 -> 166.9 us, k_update 23.2 -> 24.3 us).
-static void prepare_order(pct_ctx* c, long long block_size) {
+// (strings = 0: the DROP blocks of pct_iterate; strings = P: the blocks of the P CARP strings, which count
+// from each string's first history and work on P images at once)
+static void prepare_order(pct_ctx* c, long long block_size, int strings = 0) {
+    const double images = strings > 0 ? (double)strings : 1.0;
     const double l2 = c->l2_bytes > 0.0 ? c->l2_bytes : 128.0e6;
     // ordering pays when image + accumulator do not fit the L2; for a grid that fits it is a wash (256 x 256 x
     // 128, 101 MB: sweep 906 -> 910 ms, and every upload would pay the sort), so such grids keep the caller's
@@ -151,7 +155,7 @@ static void prepare_order(pct_ctx* c, long long block_size) {
     int mode = PCT_ORDER_BLOCKS;
     if (const char* env = getenv("PCT_ORDER"))  // tuning / test override: 0 never, 1 by footprint, 2 always
         if (env[0] >= '0' && env[0] <= '2' && env[1] == 0) mode = env[0] - '0';
-    const bool wanted = mode == 2 || (mode == 1 && 12.0 * (double)c->n_voxels > 0.85 * l2);
+    const bool wanted = mode == 2 || (mode == 1 && 12.0 * images * (double)c->n_voxels > 0.85 * l2);
     if (!wanted || block_size < 1024) {  // (small blocks: nothing to gain)
         if (c->order) cudaFree(c->order);
         c->order = nullptr;
@@ -159,14 +163,15 @@ static void prepare_order(pct_ctx* c, long long block_size) {
         return;
     }
     const double per_slab = 0.25 * l2;
-    const double want = ceil(12.0 * (double)c->n_voxels / per_slab);
+    const double want = ceil(12.0 * images * (double)c->n_voxels / per_slab);
     c->order_slabs = want < 4.0 ? 4 : (want > 64.0 ? 64 : (int)want);
-    if (c->order && c->order_block == block_size) return;
+    if (c->order && c->order_block == block_size && c->order_strings == strings) return;
     if (!c->order && cudaMalloc(&c->order, sizeof(uint32_t) * (size_t)c->n) != cudaSuccess) {
         (void)cudaGetLastError();
         c->order = nullptr;
     }
     c->order_block = block_size;
+    c->order_strings = strings;
     c->order_built = 0;
 }
 
@@ -508,6 +513,17 @@ extern "C" int pct_iterate_carp(pct_ctx* c, float lambda, int64_t block_size, in
         }
         c->carp_p = P;
     }
+    prepare_order(c, block_size, P);
+    if (c->order && c->order_built == 0) {  // every string's blocks, ordered by depth slab (k_order_blocks)
+        for (int p = 0; p < P; ++p) {
+            const long long lo = (long long)(((__int128)p * c->n) / P), hi = (long long)(((__int128)(p + 1) * c->n) / P);
+            HistPtrs Hs = c->H;
+            Hs.t_in += lo; Hs.v_in += lo; Hs.dt_in += lo; Hs.dv_in += lo;
+            CUDA_TRY(c, launch_order_blocks(Hs, c->g, hi - lo, block_size, 0, (hi - lo + block_size - 1) / block_size,
+                                            c->order_slabs, c->order + lo, c->stream));
+        }
+        c->order_built = 1;
+    }
     for (int it = 0; it < n_iter; ++it) {
         CUDA_TRY(c, cudaEventRecord(c->carp_fork, c->stream));  // x (and, the first time, the zeroed accumulators) are ready
         for (int p = 0; p < P; ++p) {
@@ -525,10 +541,13 @@ extern "C" int pct_iterate_carp(pct_ctx* c, float lambda, int64_t block_size, in
             a.x = xs;
             a.acc = c->carp_acc + (size_t)p * M;
             a.ctrl = c->carp_ctrl + p;
-            a.order = nullptr;
+            a.order = c->order ? c->order + lo : nullptr;
             const long long n_blocks = (a.n + block_size - 1) / block_size;
+            // every string gets its share of the CTA slots: P block launches in flight side by side, each P times
+            // longer (measured at 256 x 256 x 128, 1e8 histories: the same rate as whole-grid launches, 5.4e8 /s)
+            const int grid = (c->drop_grid + P - 1) / P;
             for (long long b = 0; b < n_blocks; ++b) {
-                CUDA_TRY(c, launch_drop_block(a, c->drop_grid, s));
+                CUDA_TRY(c, launch_drop_block(a, grid, s));
                 CUDA_TRY(c, launch_update(xs, a.acc, M, lambda, a.ctrl, n_blocks, s));
             }
             CUDA_TRY(c, cudaEventRecord(c->carp_done[p], s));

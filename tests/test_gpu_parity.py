@@ -276,8 +276,11 @@ def test_carp_config0(oracle_mod, pct, torch_cuda, n_strings):
     assert np.linalg.norm(x_ref) > 1.0
 
 
-def test_carp_config1_sample_from_an_image(oracle_mod, pct, torch_cuda):
-    """configs[1] geometry and block size, 3 strings of 1e5 histories, two iterations from a non-trivial image."""
+@pytest.mark.parametrize("order", ["1", "2"])
+def test_carp_config1_sample_from_an_image(oracle_mod, pct, torch_cuda, monkeypatch, order):
+    """configs[1] geometry and block size, 3 strings of 1e5 histories, two iterations from a non-trivial image;
+    order = "2" forces the depth-slab ordering of every string's blocks."""
+    monkeypatch.setenv("PCT_ORDER", order)
     cfg = synth.config(1)
     H = synth.generate_numpy(cfg, 300_000)
     _carp_parity(oracle_mod, pct, torch_cuda, cfg, H, cfg.lam, cfg.block_size, 2, 3, x0=synth.rsp_volume(cfg) * 0.8)

@@ -1,9 +1,15 @@
-"""Host logic of the N > 1 launch (replicas only).
+"""Host logic of the N > 1 launch.
 
-DROP blocks are sequential in the image, so one solve does not shard; `bench.py --gpus N` runs N
+DROP blocks are sequential in the image, so one DROP solve does not shard; `bench.py --gpus N` runs N
 independent replicas, one process per GPU, each on its own slice of the seeded history stream.  There
-is no data-path collective: the process group carries the barrier around the timed region and the
-max-over-ranks of the device time.  Backend-agnostic (nccl on the GPUs, gloo in the CPU tests).
+is no data-path collective there: the process group carries the barrier around the timed region and
+the max-over-ranks of the device time.
+
+CARP does shard ("CARP is highly suitable for parallel implementation"): one string per
+rank, and the one exchange step of the method -- "a new solution is then computed from the average of
+the different string solutions" -- is an all-reduce of the image per iteration (`carp_distributed`).
+
+Backend-agnostic (nccl on the GPUs, gloo in the CPU tests).
 """
 import torch
 import torch.distributed as dist
@@ -35,3 +41,39 @@ def whole_job_rate(ms_local, n_per_rank, steps, world, device="cpu"):
     """(ms of the slowest rank, histories * steps of ALL ranks per second of that time)."""
     ms = max_over_ranks(ms_local, world, device)
     return ms, world * int(n_per_rank) * int(steps) / (ms * 1e-3)
+
+
+def string_range(rank, world, n):
+    """CARP string of rank `rank` of `world` (R27): histories [floor(rank n / world), floor((rank + 1) n / world))."""
+    if not (0 <= rank < world) or n < world:
+        raise ValueError("0 <= rank < world <= n required")
+    return (rank * n) // world, ((rank + 1) * n) // world
+
+
+def carp_distributed(sweep, get_image, set_image, n_iter, world):
+    """n_iter CARP iterations with ONE STRING PER RANK (R27-R29).
+
+    sweep()        one DROP sweep of this rank over its own string, from the image it currently holds
+    get_image()    -> the rank's image as a tensor (on the device the process group reduces on)
+    set_image(t)   makes t the rank's image
+    Every rank starts from the same image and ends every iteration with the same one: the arithmetic mean
+    of the `world` string solutions, the all-reduce being the method's only exchange."""
+    for _ in range(int(n_iter)):
+        sweep()
+        x = get_image()
+        if world > 1:
+            dist.all_reduce(x, op=dist.ReduceOp.SUM)
+            x /= world
+        set_image(x)
+
+
+def carp_distributed_pct(pct, ctx, n_voxels, lam, block_size, n_iter, world):
+    """carp_distributed on a libpct context holding this rank's string (pct = the binding module)."""
+    buf = torch.empty(int(n_voxels), dtype=torch.float32, device="cuda")
+
+    def get_image():
+        pct.pct_get_image(ctx, buf, n_voxels)
+        return buf
+
+    carp_distributed(lambda: pct.pct_iterate(ctx, lam, block_size, 1), get_image,
+                     lambda t: pct.pct_set_image(ctx, t, n_voxels), n_iter, world)

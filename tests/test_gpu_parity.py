@@ -315,6 +315,32 @@ def test_carp_one_string_is_drop_and_arguments(pct, torch_cuda):
     assert np.linalg.norm(imgs[0] - imgs[1]) <= 1e-5 * np.linalg.norm(imgs[0])
 
 
+def test_carp_distributed_on_one_rank_is_the_drop_sweeps(pct, torch_cuda):
+    """replicas.carp_distributed_pct (one string per rank, all-reduce of the image per iteration) at world = 1:
+    get / set of the device image around every sweep must leave n_iter DROP sweeps."""
+    from paper_1707_05014_b200 import replicas
+
+    torch = torch_cuda
+    cfg = synth.config(0)
+    D = to_device(synth.generate_numpy(cfg, 20_000))
+    imgs = []
+    for dist_form in (False, True):
+        ctx = _ctx(pct, torch, cfg)
+        try:
+            pct.pct_set_histories(ctx, 20_000, D)
+            if dist_form:
+                replicas.carp_distributed_pct(pct, ctx, cfg.n_voxels, 0.5, 1000, 3, 1)
+            else:
+                pct.pct_iterate(ctx, 0.5, 1000, 3)
+            out = torch.zeros(cfg.n_voxels, dtype=torch.float32, device="cuda")
+            pct.pct_get_image(ctx, out, cfg.n_voxels)
+            imgs.append(out.cpu().numpy())
+        finally:
+            pct.pct_destroy(ctx)
+    assert np.abs(imgs[0]).max() > 0.1
+    assert np.linalg.norm(imgs[0] - imgs[1]) <= 1e-5 * np.linalg.norm(imgs[0])
+
+
 @pytest.mark.parametrize("index,n", [(3, 250_000), (4, 260_000)])
 def test_bench_launch_configuration_sample(oracle_mod, pct, torch_cuda, index, n):
     """configs[3] / configs[4] geometry with THEIR block sizes (1e5 / 2e5 histories per launch: the

@@ -76,6 +76,70 @@ def test_world_one_needs_no_process_group():
         replicas.shard_first(-1, 10)
 
 
+def _carp_worker(rank, world, port, out_dir):
+    import torch
+    import torch.distributed as dist
+
+    sys.path.insert(0, ROOT)
+    import oracle
+    import synth
+    from paper_1707_05014_b200 import replicas
+
+    os.environ["MASTER_ADDR"] = "127.0.0.1"
+    os.environ["MASTER_PORT"] = str(port)
+    dist.init_process_group("gloo", rank=rank, world_size=world)
+    try:
+        cfg = synth.config(0)
+        n, lam, B, n_iter = 6001, 0.5, 700, 2
+        H = synth.generate_numpy(cfg, n)
+        lo, hi = replicas.string_range(rank, world, n)
+        mine = {k: (v if k in ("proj_cos", "proj_sin") else v[lo:hi]) for k, v in H.items()}
+        geom = oracle.Geometry(cfg.nx, cfg.ny, cfg.nz, cfg.h, cfg.u_in, cfg.u_out)
+        hs = oracle.Histories(mine)
+        state = {"x": np.zeros(cfg.n_voxels)}
+
+        def sweep():  # the rank's local solver stands in for libpct on a GPU: one DROP sweep over its string
+            state["x"], _ = oracle.drop_iterate(geom, hs, lam, B, 1, state["x"])
+
+        replicas.carp_distributed(sweep, lambda: torch.from_numpy(state["x"].copy()),
+                                  lambda t: state.update(x=t.numpy().copy()), n_iter, world)
+        np.save(os.path.join(out_dir, "carp_%d.npy" % rank), state["x"])
+    finally:
+        dist.destroy_process_group()
+
+
+def test_carp_one_string_per_rank_equals_the_single_process_definition(tmp_path):
+    """CARP with one string per rank and an all-reduce of the image per iteration (the paper's cluster form,
+    PAPER.md:52-56) gives, on every rank, what the oracle's single-process CARP gives for P = world strings."""
+    sys.path.insert(0, ROOT)
+    import oracle
+    import synth
+
+    world, port = 2, _free_port()
+    mp.spawn(_carp_worker, args=(world, port, str(tmp_path)), nprocs=world, join=True)
+    cfg = synth.config(0)
+    H = synth.generate_numpy(cfg, 6001)
+    geom = oracle.Geometry(cfg.nx, cfg.ny, cfg.nz, cfg.h, cfg.u_in, cfg.u_out)
+    want = oracle.carp_iterate(geom, oracle.Histories(H), 0.5, 700, 2, world, np.zeros(cfg.n_voxels))
+    got = [np.load(tmp_path / ("carp_%d.npy" % r)) for r in range(world)]
+    assert np.array_equal(got[0], got[1])  # every rank ends with the same image
+    assert np.abs(want).max() > 0.1
+    assert got[0] == pytest.approx(want, abs=1e-12)
+
+
+def test_string_range_is_balanced_and_contiguous():
+    sys.path.insert(0, ROOT)
+    from paper_1707_05014_b200 import replicas
+
+    n, world = 1003, 4
+    r = [replicas.string_range(k, world, n) for k in range(world)]
+    assert r[0][0] == 0 and r[-1][1] == n
+    assert all(r[k][1] == r[k + 1][0] for k in range(world - 1))
+    assert max(b - a for a, b in r) - min(b - a for a, b in r) <= 1
+    with pytest.raises(ValueError):
+        replicas.string_range(4, 4, n)
+
+
 def test_reference_arm_under_torchrun_prints_once():
     """`bench.py --impl reference` launched as the driver launches N = 2: rank 0 runs the oracle on its
     bounded sample and prints ONE JSON line, rank 1 exits 0 without work."""

@@ -14,6 +14,7 @@ from .binding import (  # noqa: F401
     build,
     carp_iterate,
     drop_iterate,
+    get_path_model,
     lib,
     mlp_chi2_f64,
     mlp_matrix_f64,
@@ -22,6 +23,7 @@ from .binding import (  # noqa: F401
     row_f32,
     rule_log,
     scatter_f,
+    set_path_model,
     sigma1_table,
     sigma_f64,
 )

@@ -139,6 +139,9 @@ def lib():
         L.orc_carp_iterate.argtypes = [C.POINTER(_Geom), C.POINTER(_Histories), C.c_int64, C.c_double,
                                        C.c_int64, C.c_int, C.c_int, dp, C.c_int]
         L.orc_num_threads.restype = C.c_int
+        L.orc_set_path_model.argtypes = [C.c_int]
+        L.orc_set_path_model.restype = None
+        L.orc_get_path_model.restype = C.c_int
         _lib = L
     return _lib
 
@@ -268,6 +271,15 @@ def carp_iterate(geom, hists, lam, block_size, n_iter, n_strings, x, n=None, nth
     if rc:
         raise RuntimeError("orc_carp_iterate failed: %d" % rc)
     return x
+
+
+def set_path_model(model):
+    """0: most-likely path (default), 1: cubic spline through the hull points (R30).  Process-wide."""
+    lib().orc_set_path_model(int(model))
+
+
+def get_path_model():
+    return int(lib().orc_get_path_model())
 
 
 def num_threads():

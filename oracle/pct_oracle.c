@@ -229,6 +229,20 @@ typedef struct {
 /* T64 hull + MLP nodes in the object frame.  nodes: (K+2) x 3 doubles.  Returns the number of
  * nodes (K+2), 0 if the history is skipped, or -needed if max_nodes is too small.
  * hullout (optional, 7 doubles): u0,t0,v0,u2,t2,v2,L. */
+/* Path model (R30).  0: the most-likely path of the scattering-matrix
+ * formalism (the graded path).  1: the CUBIC SPLINE through the hull entry and exit points with the measured
+ * directions -- what the MLP becomes for a constant scattering power (pin P1) -- as a cheap mode:
+ *     t(s) = t0 + sigma s + c0 alpha0 + c2 alpha2,  c0 = L tau (1 - tau)^2,  c2 = -L tau^2 (1 - tau),  tau = s / L
+ * in the chord frame (alpha = direction - chord slope sigma); same for v. */
+static int g_path_model = 0;
+void orc_set_path_model(int m) { g_path_model = m == 1 ? 1 : 0; }
+int orc_get_path_model(void) { return g_path_model; }
+
+static double spline_f64(double s1, double L, const double y0[2], const double y2[2]) {
+    const double sigma = (y2[0] - y0[0]) / L, a0 = y0[1] - sigma, a2 = y2[1] - sigma, tau = s1 / L;
+    return y0[0] + sigma * s1 + L * tau * (1.0 - tau) * (1.0 - tau) * a0 - L * tau * tau * (1.0 - tau) * a2;
+}
+
 int orc_path_f64(const orc_geom *g, const orc_hist *hh, int max_nodes, double *nodes, double *hullout) {
     double h = (double)g->h;
     int nmin = g->nx < g->ny ? g->nx : g->ny;
@@ -262,10 +276,15 @@ int orc_path_f64(const orc_geom *g, const orc_hist *hh, int max_nodes, double *n
             double s1 = k * h;
             double yt0[2] = {t0, th0}, yt2[2] = {t2, th2}, yv0[2] = {v0, ph0}, yv2[2] = {v2, ph2};
             double y[2];
-            orc_mlp_matrix_f64(s1, L, yt0, yt2, NULL, 1, y);
-            t = y[0];
-            orc_mlp_matrix_f64(s1, L, yv0, yv2, NULL, 1, y);
-            v = y[0];
+            if (g_path_model == 1) {
+                t = spline_f64(s1, L, yt0, yt2);
+                v = spline_f64(s1, L, yv0, yv2);
+            } else {
+                orc_mlp_matrix_f64(s1, L, yt0, yt2, NULL, 1, y);
+                t = y[0];
+                orc_mlp_matrix_f64(s1, L, yv0, yv2, NULL, 1, y);
+                v = y[0];
+            }
             u = u0 + s1;
         }
         nodes[3 * k + 0] = t * cs - u * sn; /* rotation about z by the projection angle (R8) */
@@ -406,6 +425,16 @@ static int r32_setup(const orc_geom *g, const orc_hist *hh, r32_state *st) {
 static void r32_coef(const r32_state *st, float h, int k, const float *p11t, const float *p12t,
                      const float *p22t, float *s1_out, float *c0_out, float *c2_out) {
     const float s1 = (float)k * h;
+    if (g_path_model == 1) { /* spline rule (R30): five fp32 operations after tau = s1 * (1/L) */
+        const float invL = 1.0f / st->L;
+        const float tau = s1 * invL;
+        const float om = 1.0f - tau;
+        const float a = tau * om;
+        *s1_out = s1;
+        *c0_out = (a * om) * st->L;
+        *c2_out = -((a * tau) * st->L);
+        return;
+    }
     const float d = st->L - s1;
     const float p11 = p11t[k], p12 = p12t[k], p22 = p22t[k];
     const float e1 = fmaf(p11, s1, p12);

@@ -7,6 +7,8 @@ from ._build import build  # noqa: F401
 from .binding import (  # noqa: F401
     EXPORTS,
     FIELDS,
+    PCT_PATH_MLP,
+    PCT_PATH_SPLINE,
     PctError,
     lib,
     pct_create,
@@ -21,6 +23,7 @@ from .binding import (  # noqa: F401
     pct_set_histories,
     pct_set_histories_host,
     pct_set_image,
+    pct_set_path_model,
     pct_synchronize,
     pct_version,
 )

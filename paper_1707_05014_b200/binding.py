@@ -47,6 +47,7 @@ def lib():
         L.pct_set_histories_host.argtypes = [vp, i64, C.POINTER(pct_histories)]
         L.pct_iterate.argtypes = [vp, C.c_float, i64, C.c_int]
         L.pct_iterate_carp.argtypes = [vp, C.c_float, i64, C.c_int, C.c_int]
+        L.pct_set_path_model.argtypes = [vp, C.c_int]
         L.pct_get_image.argtypes = [vp, vp, i64]
         L.pct_set_image.argtypes = [vp, vp, i64]
         L.pct_synchronize.argtypes = [vp]
@@ -63,7 +64,7 @@ def lib():
     return _lib
 
 
-EXPORTS = ("pct_create", "pct_set_histories", "pct_set_histories_host", "pct_iterate", "pct_iterate_carp", "pct_get_image",
+EXPORTS = ("pct_create", "pct_set_histories", "pct_set_histories_host", "pct_iterate", "pct_iterate_carp", "pct_set_path_model", "pct_get_image",
            "pct_set_image", "pct_synchronize", "pct_get_stats", "pct_destroy", "pct_last_error", "pct_version",
            "pct_debug_rows", "pct_debug_block", "pct_profile_sweep")
 
@@ -125,6 +126,13 @@ def pct_iterate(ctx, lam, block_size, n_iter):
 
 def pct_iterate_carp(ctx, lam, block_size, n_iter, n_strings):
     _check(ctx, lib().pct_iterate_carp(ctx, float(lam), int(block_size), int(n_iter), int(n_strings)))
+
+
+PCT_PATH_MLP, PCT_PATH_SPLINE = 0, 1
+
+
+def pct_set_path_model(ctx, model):
+    _check(ctx, lib().pct_set_path_model(ctx, int(model)))
 
 
 def pct_get_image(ctx, dst, n_voxels):

@@ -558,6 +558,16 @@ extern "C" int pct_iterate_carp(pct_ctx* c, float lambda, int64_t block_size, in
     return PCT_OK;
 }
 
+extern "C" int pct_set_path_model(pct_ctx* c, int model) {
+    if (!c) return PCT_EINVAL;
+    if (model != PCT_PATH_MLP && model != PCT_PATH_SPLINE) return fail(c, PCT_EINVAL, "pct_set_path_model: unknown model");
+    if (c->g.path_model != model) {
+        c->g.path_model = model;
+        drop_graph(c);  // the cached graph holds the kernel of the other model
+    }
+    return PCT_OK;
+}
+
 extern "C" int pct_synchronize(pct_ctx* c) {
     if (!c) return PCT_EINVAL;
     if (int rc = wait_upload(c, -1)) return rc;  // the host arrays are free once this returns

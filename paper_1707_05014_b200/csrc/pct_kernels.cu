@@ -186,10 +186,11 @@ __device__ __forceinline__ Node2 pair3(const float3 a, const float3 b) {
 
 // Nodes k and k+1 of the path (rule step 3), both halves of one packed evaluation; a node past the
 // last interior one is the hull exit point (R9).  k <= 0 gives an unspecified (unused) first half.
+template <bool SPLINE>
 __device__ __forceinline__ Node2 node_pair(const PathState& st, const float4* s_tab, const float4* s_tabB, int pad_mask, int k,
                                            int K, const float3 exitP) {
     const int slot = k + ((k >> 3) & pad_mask);  // padded copy: tab_slot(k); plain copy: k
-    const Node2 n = mlp_node2(st, s_tab[slot], s_tabB[slot]);
+    const Node2 n = mlp_node2<SPLINE>(st, s_tab[slot], s_tabB[slot]);
     float3 a = lo3(n), b = hi3(n);
     if (k > K) a = exitP;
     if (k + 1 > K) b = exitP;
@@ -218,7 +219,7 @@ __device__ __forceinline__ void take_two(const Geom& g, const Node2& a, const No
 // the one or two segments that end at the nodes it evaluated first.  The MLP node at depth k*h is
 // closed-form in k, there is no recurrence along the path.  Lanes past the end of the path run the
 // same instructions on harmless values and are masked.
-template <bool EMIT>
+template <bool EMIT, bool SPLINE>
 __device__ __forceinline__ void walk_history(const Geom& g, const PathState& S, const float4* s_tab, int lane, float2* row,
                                              float& nrm, int& nnz, const EmitPtrs& em) {
     const PathState st = S;  // shared memory -> registers, once per history
@@ -230,7 +231,7 @@ __device__ __forceinline__ void walk_history(const Geom& g, const PathState& S, 
     const float4* s_tabB = s_tabA + tab_n;
     const int k0 = lane * C;
     const float3 exitP = to_object(st, st.t2, st.u2, st.v2);  // node K+1: the hull exit point, assigned (R9)
-    const Node2 Z = node_pair(st, s_tabA, s_tabB, pad_mask, k0 + C - 1, K, exitP);
+    const Node2 Z = node_pair<SPLINE>(st, s_tabA, s_tabB, pad_mask, k0 + C - 1, K, exitP);
     const float3 last = hi3(Z);
     float3 prv;
     prv.x = __shfl_up_sync(0xffffffffu, last.x, 1);
@@ -242,7 +243,7 @@ __device__ __forceinline__ void walk_history(const Geom& g, const PathState& S, 
     int c = 1;  // next node of the lane to evaluate; segments k0 .. k0+c-2 are done
 #pragma unroll kWalkUnroll
     for (; c <= C - 2; c += 2) {
-        const Node2 N = node_pair(st, s_tabA, s_tabB, pad_mask, k0 + c, K, exitP);
+        const Node2 N = node_pair<SPLINE>(st, s_tabA, s_tabB, pad_mask, k0 + c, K, exitP);
         take_two<EMIT>(g, pair3(prv, lo3(N)), N, k0 + c - 1, true, K, m, row_sa, em);
         prv = hi3(N);
     }
@@ -465,6 +466,7 @@ __device__ __forceinline__ void queue_item(const Queue& q, unsigned long long w,
     cnt = left < q.size[p] ? (int)left : q.size[p];
 }
 
+template <bool SPLINE>
 __global__ void __launch_bounds__(kThreads, kCtasPerSm) k_drop_block(const DropArgs a) {
     extern __shared__ __align__(16) unsigned char smem_raw[];
     const Geom g = a.g;
@@ -511,7 +513,7 @@ __global__ void __launch_bounds__(kThreads, kCtasPerSm) k_drop_block(const DropA
             if (K < 0) continue;  // skipped history: empty row (R7)
             float nrm;
             int nnz;
-            walk_history<false>(g, S, s_tab, lane, row, nrm, nnz, no_emit);
+            walk_history<false, SPLINE>(g, S, s_tab, lane, row, nrm, nnz, no_emit);
             const int C = (K + 32) >> 5;
             float dot = gather_row(row, lane, C, a.x);
             dot = warp_sum(dot);
@@ -542,8 +544,9 @@ cudaError_t drop_configure(int nmin, int* grid_out) {
     cudaError_t e;
     if ((e = cudaGetDevice(&dev)) != cudaSuccess) return e;
     if ((e = cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev)) != cudaSuccess) return e;
-    e = cudaFuncSetAttribute(k_drop_block, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-    if (e == cudaSuccess) e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, k_drop_block, kThreads, smem);
+    e = cudaFuncSetAttribute(k_drop_block<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(k_drop_block<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    if (e == cudaSuccess) e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, k_drop_block<false>, kThreads, smem);
     if (e != cudaSuccess) return e;
     if (per_sm < 1) return cudaErrorLaunchOutOfResources;
     *grid_out = sms * per_sm;  // persistent: every CTA slot of the chip, work handed out dynamically
@@ -556,7 +559,10 @@ cudaError_t launch_drop_block(const DropArgs& a, int grid, cudaStream_t stream) 
     const long long need = (cnt + kWarpsPerCta - 1) / kWarpsPerCta;
     if (need < grid) grid = need < 1 ? 1 : (int)need;
     const size_t smem = drop_smem_bytes(a.g.nmin);
-    k_drop_block<<<grid, kThreads, smem, stream>>>(a);
+    if (a.g.path_model == 1)
+        k_drop_block<true><<<grid, kThreads, smem, stream>>>(a);
+    else
+        k_drop_block<false><<<grid, kThreads, smem, stream>>>(a);
     return cudaGetLastError();
 }
 
@@ -686,6 +692,7 @@ cudaError_t launch_split_acc(float2* acc, float* delta, float* cnt, long long n,
 // the run heads and the non-zero count are those of the hot path; only the merged length of a
 // run (which the hot path never forms: it needs ||a_i||^2 and the unmerged scatter only) is
 // summed here, from the segment lengths just written.
+template <bool SPLINE>
 __global__ void __launch_bounds__(kThreads) k_rows(const RowsArgs a) {
     extern __shared__ __align__(16) unsigned char smem_raw[];
     const Geom g = a.g;
@@ -712,7 +719,7 @@ __global__ void __launch_bounds__(kThreads) k_rows(const RowsArgs a) {
             em.nodes = a.nodes ? a.nodes + (size_t)r * (a.max_seg + 1) * 3 : nullptr;
             float nrm;
             int nnz;
-            walk_history<true>(g, S, s_tab, lane, row, nrm, nnz, em);
+            walk_history<true, SPLINE>(g, S, s_tab, lane, row, nrm, nnz, em);
             nnz_total = __reduce_add_sync(0xffffffffu, nnz);
             // the row as the hot path sees it: read back from the row buffer, segment-major
             for (int k = lane; k <= K; k += 32) {
@@ -748,8 +755,13 @@ cudaError_t launch_rows(const RowsArgs& a, cudaStream_t stream) {
     if (blocks > 148 * 8) blocks = 148 * 8;
     if (blocks < 1) blocks = 1;
     cudaError_t e = cudaSuccess;
-    e = cudaFuncSetAttribute(k_rows, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-    if (e == cudaSuccess) k_rows<<<(int)blocks, kThreads, smem, stream>>>(a);
+    if (a.g.path_model == 1) {
+        e = cudaFuncSetAttribute(k_rows<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+        if (e == cudaSuccess) k_rows<true><<<(int)blocks, kThreads, smem, stream>>>(a);
+    } else {
+        e = cudaFuncSetAttribute(k_rows<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+        if (e == cudaSuccess) k_rows<false><<<(int)blocks, kThreads, smem, stream>>>(a);
+    }
     if (e != cudaSuccess) return e;
     return cudaGetLastError();
 }

@@ -341,6 +341,76 @@ def test_carp_distributed_on_one_rank_is_the_drop_sweeps(pct, torch_cuda):
     assert np.linalg.norm(imgs[0] - imgs[1]) <= 1e-5 * np.linalg.norm(imgs[0])
 
 
+@pytest.fixture()
+def spline_oracle(oracle_mod):
+    oracle_mod.set_path_model(1)
+    yield oracle_mod
+    oracle_mod.set_path_model(0)
+
+
+def test_spline_path_model_rows_and_run(spline_oracle, pct, torch_cuda):
+    """PCT_PATH_SPLINE (NEXT-3, R30) against the oracle in the same mode: voxel sequences bit-exact on configs[0]
+    and on configs[3] geometry, a full DROP run and a CARP run within the DROP tolerances; and switching back to
+    the most-likely path gives the default rows again."""
+    torch = torch_cuda
+    oracle = spline_oracle
+    for index, n in ((0, 4000), (3, 1500)):
+        cfg = synth.config(index)
+        H = synth.generate_numpy(cfg, n)
+        geom = oracle_geom(oracle, cfg)
+        hs = oracle.Histories(H)
+        table = oracle.sigma1_table(geom.h, geom.nmin)
+        ctx = _ctx(pct, torch, cfg)
+        D = to_device(H)  # borrowed by the library: kept alive until pct_destroy
+        try:
+            pct.pct_set_histories(ctx, n, D)
+            default = _gpu_rows(pct, torch, ctx, 0, n, geom.nmin)
+            pct.pct_set_path_model(ctx, pct.PCT_PATH_SPLINE)
+            nseg, nnz, seg_idx, seg_len, row_len, nodes = _gpu_rows(pct, torch, ctx, 0, n, geom.nmin)
+            differ = 0
+            for i in range(n):
+                r = oracle.row_f32(geom, hs.hist(i), table)
+                assert nseg[i] == r["nseg"] and nnz[i] == r["nnz"], i
+                assert np.array_equal(seg_idx[i, :r["nseg"]], r["seg_idx"]), i
+                if r["nseg"]:
+                    assert np.array_equal(nodes[i, :r["nseg"] + 1], r["nodes"]), i  # fp32 node positions: bitwise
+                differ += int(not np.array_equal(seg_idx[i], default[2][i]))
+            assert differ > 0  # the two models do walk different voxels now and then
+            pct.pct_set_path_model(ctx, pct.PCT_PATH_MLP)
+            again = _gpu_rows(pct, torch, ctx, 0, n, geom.nmin)
+            assert np.array_equal(again[2], default[2])
+            with pytest.raises(pct.PctError):
+                pct.pct_set_path_model(ctx, 7)
+        finally:
+            pct.pct_destroy(ctx)
+    # full runs in spline mode
+    cfg = synth.config(0)
+    H = synth.generate_numpy(cfg, 30_011)
+    geom = oracle_geom(oracle, cfg)
+    hs = oracle.Histories(H)
+    M = cfg.n_voxels
+    ctx = _ctx(pct, torch, cfg)
+    out = torch.zeros(M, dtype=torch.float32, device="cuda")
+    D = to_device(H)
+    try:
+        pct.pct_set_histories(ctx, hs.n, D)
+        pct.pct_set_path_model(ctx, pct.PCT_PATH_SPLINE)
+        x_ref = np.zeros(M)
+        for it in range(3):
+            if it < 2:
+                pct.pct_iterate(ctx, 0.5, 700, 1)
+                x_ref, _ = oracle.drop_iterate(geom, hs, 0.5, 700, 1, x_ref)
+            else:
+                pct.pct_iterate_carp(ctx, 0.5, 700, 1, 3)
+                x_ref = oracle.carp_iterate(geom, hs, 0.5, 700, 1, 3, x_ref)
+            pct.pct_get_image(ctx, out, M)
+            x = out.cpu().numpy().astype(np.float64)
+            assert np.linalg.norm(x - x_ref) <= REL_L2_PER_ITER * np.linalg.norm(x_ref)
+        assert np.abs(x - x_ref).max() <= ABS_FINAL
+    finally:
+        pct.pct_destroy(ctx)
+
+
 @pytest.mark.parametrize("index,n", [(3, 250_000), (4, 260_000)])
 def test_bench_launch_configuration_sample(oracle_mod, pct, torch_cuda, index, n):
     """configs[3] / configs[4] geometry with THEIR block sizes (1e5 / 2e5 histories per launch: the

@@ -57,6 +57,8 @@ def parse_args():
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu", action="store_true")
     ap.add_argument("--cpu-seconds", type=float, default=15.0, help="target CPU time of the oracle sample")
+    ap.add_argument("--path-model", default="mlp", choices=["mlp", "spline"],
+                    help="spline: the cubic-spline path model (SURVEY.md 8(f) NEXT-3), a side measurement; the metric's is mlp")
     ap.add_argument("--carp-strings", type=int, default=0,
                     help="P > 0: time pct_iterate_carp with P strings instead of the metric's DROP sweep (SURVEY.md 8(f) NEXT-1; "
                          "a side measurement: one short JSON line, not the driver's contract)")
@@ -228,6 +230,7 @@ def run_ours(args):
     with torch.cuda.stream(stream):  # torch.cuda.Event records on this stream, the one the kernels run on
         ctx = pct.pct_create(cfg.nx, cfg.ny, cfg.nz, cfg.h, cfg.u_in, cfg.u_out, stream.cuda_stream)
         try:
+            pct.pct_set_path_model(ctx, pct.PCT_PATH_SPLINE if args.path_model == "spline" else pct.PCT_PATH_MLP)
             pct.pct_set_histories(ctx, n, P)
             for _ in range(args.warmup):
                 pct.pct_iterate(ctx, lam, B, 1)
@@ -269,6 +272,7 @@ def run_ours(args):
             img_host = torch.empty(M, dtype=torch.float32, pin_memory=True)
             ctx = pct.pct_create(cfg.nx, cfg.ny, cfg.nz, cfg.h, cfg.u_in, cfg.u_out, stream.cuda_stream)
             try:
+                pct.pct_set_path_model(ctx, pct.PCT_PATH_SPLINE if args.path_model == "spline" else pct.PCT_PATH_MLP)
                 host_ms = [0.0, 0.0, 0.0]  # host clock: upload enqueue (+ device allocation), sweep enqueue, wait + D2H
 
                 def e2e_step():
@@ -359,7 +363,9 @@ def run_ours(args):
                    "step": "one DROP sweep (iteration) over all histories",
                    "l2": "inputs larger than L2 (histories %.1f GB, image+accumulator %.0f MB vs 126 MB L2)" % (
                        38.0 * n / 1e9, 12.0 * M / 1e6),
-                   "multi_gpu": "replicas only", "histories_override": args.histories is not None},
+                   "multi_gpu": "replicas only", "histories_override": args.histories is not None,
+                   "path_model": "most-likely path (the metric's)" if args.path_model == "mlp"
+                   else "cubic spline (side measurement, SURVEY.md 8(f) NEXT-3; the roofline's op count is the MLP's)"},
         "clocks": out["clocks"], "gpu_launches": 2 * n_blocks * args.steps,
         "segments_per_history": seg_per_hist, "nonzeros_per_history": nnz_per_hist,
         "skipped_fraction": 1.0 - st["rows"] / max(1, st["histories"]),

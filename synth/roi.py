@@ -49,7 +49,7 @@ def markdown(rows):
     return "\n".join(out)
 
 
-def reconstruct(cfg, n, n_iter, carp_strings=0):
+def reconstruct(cfg, n, n_iter, carp_strings=0, spline=False):
     """The reconstruction of cfg's first n histories on cuda:0 through the C ABI -> image (numpy float32)."""
     import torch
 
@@ -61,6 +61,7 @@ def reconstruct(cfg, n, n_iter, carp_strings=0):
     ctx = pct.pct_create(cfg.nx, cfg.ny, cfg.nz, cfg.h, cfg.u_in, cfg.u_out, torch.cuda.current_stream().cuda_stream)
     try:
         pct.pct_set_histories(ctx, n, D)
+        pct.pct_set_path_model(ctx, pct.PCT_PATH_SPLINE if spline else pct.PCT_PATH_MLP)
         if carp_strings > 0:
             pct.pct_iterate_carp(ctx, cfg.lam, cfg.block_size, n_iter, carp_strings)
         else:
@@ -78,18 +79,19 @@ def main():
     ap.add_argument("--histories", type=float, default=None)
     ap.add_argument("--iterations", type=int, default=None)
     ap.add_argument("--carp-strings", type=int, default=0)
+    ap.add_argument("--spline", action="store_true", help="cubic-spline path model instead of the most-likely path")
     ap.add_argument("--json", action="store_true")
     a = ap.parse_args()
     cfg = config(a.config)
     n = cfg.n if a.histories is None else int(a.histories)
     it = cfg.n_iter if a.iterations is None else a.iterations
-    img = reconstruct(cfg, n, it, a.carp_strings)
+    img = reconstruct(cfg, n, it, a.carp_strings, a.spline)
     rows = roi_table(cfg, img)
     truth = rsp_volume(cfg)
     hull = truth > 10 * AIR
     rms = float(np.sqrt(np.mean((img[hull] - truth[hull]) ** 2)))
     head = "%s, %d histories, %d iterations, %s, lambda %.3g, block %d; RMS error inside the object %.4f" % (
-        cfg.workload, n, it, "CARP with %d strings" % a.carp_strings if a.carp_strings else "DROP", cfg.lam, cfg.block_size, rms)
+        cfg.workload, n, it, ("CARP with %d strings" % a.carp_strings if a.carp_strings else "DROP") + (", spline path" if a.spline else ", most-likely path"), cfg.lam, cfg.block_size, rms)
     if a.json:
         print(json.dumps(dict(run=head, rows=rows, rms=rms)))
     else:

@@ -19,6 +19,7 @@ from .binding import (  # noqa: F401
     pct_get_stats,
     pct_iterate,
     pct_iterate_carp,
+    pct_measure_peaks,
     pct_profile_sweep,
     pct_set_histories,
     pct_set_histories_host,

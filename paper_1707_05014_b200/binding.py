@@ -37,9 +37,9 @@ def lib():
     """Load (building first if needed) libpct.so.  Raises if that is impossible -- no fallback."""
     global _lib
     if _lib is None:
-        path = _build.LIB
-        if not os.path.exists(path) or os.environ.get("PCT_REBUILD"):
-            path = _build.build()
+        # always through the stamp check (a cheap no-op when sources and flags are unchanged): a stale
+        # binary next to newer sources is rebuilt, never silently loaded
+        path = _build.build(force=bool(os.environ.get("PCT_REBUILD")))
         L = C.CDLL(path)
         vp, i64 = C.c_void_p, C.c_int64
         L.pct_create.argtypes = [C.POINTER(vp), C.c_int, C.c_int, C.c_int, C.c_float, C.c_float, C.c_float, vp]
@@ -60,13 +60,14 @@ def lib():
         L.pct_debug_rows.argtypes = [vp, i64, i64, C.c_int32, vp, vp, vp, vp, vp, vp]
         L.pct_debug_block.argtypes = [vp, i64, i64, vp, vp]
         L.pct_profile_sweep.argtypes = [vp, C.c_float, i64, C.POINTER(C.c_float)]
+        L.pct_measure_peaks.argtypes = [vp, i64, C.POINTER(C.c_double)]
         _lib = L
     return _lib
 
 
 EXPORTS = ("pct_create", "pct_set_histories", "pct_set_histories_host", "pct_iterate", "pct_iterate_carp", "pct_set_path_model", "pct_get_image",
            "pct_set_image", "pct_synchronize", "pct_get_stats", "pct_destroy", "pct_last_error", "pct_version",
-           "pct_debug_rows", "pct_debug_block", "pct_profile_sweep")
+           "pct_debug_rows", "pct_debug_block", "pct_profile_sweep", "pct_measure_peaks")
 
 
 def _ptr(a):
@@ -171,3 +172,13 @@ def pct_profile_sweep(ctx, lam, block_size):
     out = (C.c_float * 4)()
     _check(ctx, lib().pct_profile_sweep(ctx, float(lam), int(block_size), out))
     return dict(accumulate_ms=out[0], update_ms=out[1], sweep_ms=out[2], blocks=int(out[3]))
+
+
+def pct_measure_peaks(footprint_bytes, cuda_stream=None):
+    """Micro-benchmarks behind the roofline (include/pct.h: pct_measure_peaks) -> dict."""
+    out = (C.c_double * 8)()
+    rc = lib().pct_measure_peaks(cuda_stream, int(footprint_bytes), out)
+    if rc != PCT_OK:
+        raise PctError(rc, "pct_measure_peaks failed")
+    return dict(gather_random_per_s=out[0], gather_path_per_s=out[1], red_v2_random_per_s=out[2], stream_read_bytes_per_s=out[3],
+                ffma_inst_per_s=out[4], ffma2_inst_per_s=out[5], red_v2_path_per_s=out[6], footprint_bytes=int(out[7]))

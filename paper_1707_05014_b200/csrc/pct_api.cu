@@ -6,6 +6,8 @@
 #include <stdlib.h>
 #include <string.h>
 
+#include <stddef.h>
+
 #include <new>
 #include <vector>
 
@@ -13,6 +15,16 @@
 #include "pct_internal.h"
 
 using namespace pct;
+
+// Plan of the DROP blocks of one string of histories (the whole set for pct_iterate): where k_plan_blocks put its
+// results and how far it has got (blocks are planned as their histories arrive, include/pct.h pct_set_histories_host).
+struct WavePlan {
+    long long first = 0, n = 0;  // histories [first, first + n) of the context's set
+    long long n_blocks = 0, built = 0;
+    uint32_t* plan = nullptr;    // = plan_buf + first (borrowed)
+    int* need = nullptr;         // owned: [n_blocks][n_slabs]
+    int* done = nullptr;         // owned: [n_blocks][n_slabs]
+};
 
 struct pct_ctx {
     int device = 0;
@@ -55,6 +67,18 @@ struct pct_ctx {
     std::vector<cudaStream_t> carp_stream;
     std::vector<cudaEvent_t> carp_done;
     cudaEvent_t carp_fork = nullptr;
+    // wavefront engine (pct_wave.cu): the default; PCT_ENGINE=blocks selects the launch-pair-per-block engine
+    int engine = 1;
+    int sm_count = 148;
+    int wave_grid = 0;
+    WaveShape shape{};
+    WaveCtrl* wctrl = nullptr;
+    uint32_t* plan_buf = nullptr;  // 4 B per history: processing order + slab range of every history (k_plan_blocks)
+    long long plan_block = 0;      // block size the plans were made for
+    int plan_strings = -1;         // 0: pct_iterate's blocks, P: the blocks of P CARP strings
+    std::vector<WavePlan> plans;   // one per string (one for DROP)
+    WaveCtrl* carp_wctrl = nullptr;
+    long long carp_stride = 0;     // voxels between the images / accumulators of two strings (a multiple of four)
     // cached CUDA graph of kGraphPairs (accumulate, update) pairs
     cudaGraphExec_t graph = nullptr;
     float graph_lambda = 0.f;
@@ -77,6 +101,17 @@ static int fail(pct_ctx* c, int code, const char* fmt, const char* detail = "") 
     snprintf(dst, 512, fmt, detail);
     return code;
 }
+// Every entry point runs on the context's device, whatever device the calling thread has current, and restores it.
+struct DeviceGuard {
+    int prev = -1;
+    bool switched = false;
+    explicit DeviceGuard(int dev) {
+        if (cudaGetDevice(&prev) == cudaSuccess && prev != dev) switched = cudaSetDevice(dev) == cudaSuccess;
+    }
+    ~DeviceGuard() {
+        if (switched) cudaSetDevice(prev);
+    }
+};
 #define CUDA_TRY(c, call)                                                                  \
     do {                                                                                   \
         cudaError_t e__ = (call);                                                          \
@@ -183,8 +218,21 @@ static int build_order(pct_ctx* c, long long block_size, long long upto) {
     return PCT_OK;
 }
 
+static void release_plans(pct_ctx* c) {
+    for (WavePlan& pl : c->plans) {
+        if (pl.need) cudaFree(pl.need);
+        if (pl.done) cudaFree(pl.done);
+    }
+    c->plans.clear();
+    c->plan_block = 0;
+    c->plan_strings = -1;
+}
+
 static void release_histories(pct_ctx* c) {
     drop_graph(c);
+    release_plans(c);
+    if (c->plan_buf) cudaFree(c->plan_buf);
+    c->plan_buf = nullptr;
     if (c->order) cudaFree(c->order);
     c->order = nullptr;
     c->order_block = 0;
@@ -216,7 +264,7 @@ extern "C" int pct_create(pct_ctx** out, int nx, int ny, int nz, float h, float 
     if ((long long)nx * ny * nz >= (1LL << 31)) return fail(nullptr, PCT_EINVAL, "pct_create: nx*ny*nz must be < 2^31");
     if (!(h > 0.0f) || !isfinite(h)) return fail(nullptr, PCT_EINVAL, "pct_create: voxel_mm must be positive and finite");
     const int nmin = nx < ny ? nx : ny;
-    if (nmin > 4096) return fail(nullptr, PCT_EINVAL, "pct_create: min(nx,ny) must be <= 4096");
+    if (nmin > 2016) return fail(nullptr, PCT_EINVAL, "pct_create: min(nx,ny) must be <= 2016 (64 path segments per lane)");
     // rule step G (fp32, this operation order)
     Geom g{};
     g.nx = nx; g.ny = ny; g.nz = nz; g.nmin = nmin;
@@ -256,7 +304,21 @@ extern "C" int pct_create(pct_ctx** out, int nx, int ny, int nz, float h, float 
         if (e == cudaSuccess) e = cudaStreamSynchronize(c->stream);
         free(tab);
         CUDA_TRY(nullptr, e);
+        CUDA_TRY(nullptr, cudaDeviceGetAttribute(&c->sm_count, cudaDevAttrMultiProcessorCount, c->device));
+        CUDA_TRY(nullptr, cudaMalloc(&c->wctrl, sizeof(WaveCtrl)));
+        CUDA_TRY(nullptr, cudaMemsetAsync(c->wctrl, 0, sizeof(WaveCtrl), c->stream));
+        c->shape = wave_shape(g);
+        if (const char* env = getenv("PCT_ENGINE")) c->engine = strcmp(env, "blocks") == 0 ? 0 : 1;
+        // the per-warp row buffer and the two staged copies of the table must fit the shared memory of an SM
+        int smem_max = 0;
+        CUDA_TRY(nullptr, cudaDeviceGetAttribute(&smem_max, cudaDevAttrMaxSharedMemoryPerBlockOptin, c->device));
+        if (drop_smem_bytes(nmin) > (size_t)smem_max) {
+            snprintf(g_create_err, 512, "pct_create: min(nx,ny) = %d needs %zu B of shared memory per CTA, the device offers %d",
+                     nmin, drop_smem_bytes(nmin), smem_max);
+            return PCT_EINVAL;
+        }
         CUDA_TRY(nullptr, drop_configure(nmin, &c->drop_grid));
+        CUDA_TRY(nullptr, wave_configure(nmin, &c->wave_grid));
         return PCT_OK;
     };
     rc = body();
@@ -284,6 +346,8 @@ static void release_carp(pct_ctx* c) {
     if (c->carp_x) cudaFree(c->carp_x);
     if (c->carp_acc) cudaFree(c->carp_acc);
     if (c->carp_ctrl) cudaFree(c->carp_ctrl);
+    if (c->carp_wctrl) cudaFree(c->carp_wctrl);
+    c->carp_wctrl = nullptr;
     c->carp_x = nullptr;
     c->carp_acc = nullptr;
     c->carp_ctrl = nullptr;
@@ -300,6 +364,7 @@ extern "C" void pct_destroy(pct_ctx* c) {
     if (c->acc) cudaFree(c->acc);
     if (c->tab) cudaFree(c->tab);
     if (c->ctrl) cudaFree(c->ctrl);
+    if (c->wctrl) cudaFree(c->wctrl);
     (void)cudaGetLastError();
     delete c;
 }
@@ -332,6 +397,7 @@ static int check_histories(pct_ctx* c, long long n, const pct_histories* h, bool
 extern "C" int pct_set_histories(pct_ctx* c, int64_t n, const pct_histories* h) {
     int rc = check_histories(c, n, h, true);
     if (rc) return rc;
+    DeviceGuard guard(c->device);
     release_histories(c);
     CUDA_TRY(c, cudaMalloc(&c->tables, sizeof(float) * 2 * h->n_proj));
     CUDA_TRY(c, cudaMemcpyAsync(c->tables, h->proj_cos, sizeof(float) * h->n_proj, cudaMemcpyDeviceToDevice, c->stream));
@@ -343,9 +409,25 @@ extern "C" int pct_set_histories(pct_ctx* c, int64_t n, const pct_histories* h) 
     return PCT_OK;
 }
 
+static int set_histories_host_impl(pct_ctx* c, int64_t n, const pct_histories* h);
+
 extern "C" int pct_set_histories_host(pct_ctx* c, int64_t n, const pct_histories* h) {
     int rc = check_histories(c, n, h, false);
     if (rc) return rc;
+    DeviceGuard guard(c->device);
+    rc = set_histories_host_impl(c, n, h);
+    if (rc != PCT_OK) {  // a failure part-way (allocation, a copy that could not be enqueued) leaves NO histories set
+        char keep[512];
+        memcpy(keep, c->err, 512);
+        if (c->copy_stream) cudaStreamSynchronize(c->copy_stream);
+        release_histories(c);
+        (void)cudaGetLastError();
+        memcpy(c->err, keep, 512);
+    }
+    return rc;
+}
+
+static int set_histories_host_impl(pct_ctx* c, int64_t n, const pct_histories* h) {
     // one owned block: 9 float arrays (each padded to 256 B) + the uint16 array
     const size_t fa = ((sizeof(float) * (size_t)n + 255) / 256) * 256;
     const size_t total = 9 * fa + ((sizeof(uint16_t) * (size_t)n + 255) / 256) * 256;
@@ -359,6 +441,7 @@ extern "C" int pct_set_histories_host(pct_ctx* c, int64_t n, const pct_histories
         c->chunk_end.clear();
         c->chunks_waited = 0;
         c->order_built = 0;  // same buffer, new histories: the blocks are ordered again as they arrive
+        for (WavePlan& pl : c->plans) pl.built = 0;  // and planned again
         cudaEvent_t tail = nullptr;
         CUDA_TRY(c, cudaEventCreateWithFlags(&tail, cudaEventDisableTiming));
         cudaError_t e = cudaEventRecord(tail, c->stream);
@@ -422,6 +505,143 @@ static int enqueue_pair(pct_ctx* c, const DropArgs& a, float lambda, long long n
     return PCT_OK;
 }
 
+
+// ---- wavefront engine: plans and sweeps (pct_wave.cu) ----------------------------------------------------------
+
+static HistPtrs offset_hist(HistPtrs H, long long lo) {
+    H.t_in += lo; H.v_in += lo; H.t_out += lo; H.v_out += lo;
+    H.dt_in += lo; H.dv_in += lo; H.dt_out += lo; H.dv_out += lo;
+    H.wepl += lo; H.proj += lo;
+    return H;
+}
+
+// The plans of the DROP blocks of `strings` strings (0: one plan over all histories; P: the P strings of CARP,
+// string p = histories [floor(p n / P), floor((p+1) n / P)), blocks counted from the string's first history, R27).
+static int ensure_plans(pct_ctx* c, long long block_size, int strings) {
+    if (!c->plans.empty() && c->plan_block == block_size && c->plan_strings == strings) return PCT_OK;
+    release_plans(c);
+    if (!c->plan_buf) CUDA_TRY(c, cudaMalloc(&c->plan_buf, sizeof(uint32_t) * (size_t)c->n));
+    const int P = strings > 0 ? strings : 1;
+    c->plans.resize(P);
+    for (int p = 0; p < P; ++p) {
+        WavePlan& pl = c->plans[p];
+        const long long lo = (long long)(((__int128)p * c->n) / P), hi = (long long)(((__int128)(p + 1) * c->n) / P);
+        pl.first = lo;
+        pl.n = hi - lo;
+        pl.n_blocks = (pl.n + block_size - 1) / block_size;
+        pl.built = 0;
+        pl.plan = c->plan_buf + lo;
+        const size_t cells = (size_t)pl.n_blocks * c->shape.n_slabs;
+        cudaError_t e = cudaMalloc(&pl.need, sizeof(int) * cells);
+        if (e == cudaSuccess) e = cudaMalloc(&pl.done, sizeof(int) * cells);
+        if (e != cudaSuccess) {
+            release_plans(c);
+            CUDA_TRY(c, e);
+        }
+    }
+    c->plan_block = block_size;
+    c->plan_strings = strings;
+    return PCT_OK;
+}
+
+// Plan blocks [built, upto) of the string (their histories must be on the device or on their way in stream order).
+static int build_plan(pct_ctx* c, WavePlan& pl, long long block_size, long long upto, cudaStream_t s) {
+    if (upto <= pl.built) return PCT_OK;
+    CUDA_TRY(c, launch_plan_blocks(offset_hist(c->H, pl.first), c->g, pl.n, block_size, pl.built, upto - pl.built, c->shape, pl.plan,
+                                   pl.need, s));
+    pl.built = upto;
+    return PCT_OK;
+}
+
+// Histories per work item: small enough that the items in flight (one per warp) cover well under a block, so that a
+// warp drawing the first item of block q+1 finds the first slabs of block q long updated (PCT_WAVE_ITEM overrides).
+static int wave_item(long long block_size, int grid) {
+    if (const char* env = getenv("PCT_WAVE_ITEM")) {
+        const int v = atoi(env);
+        if (v >= 1 && v <= 16) return v;
+    }
+    const long long warps = (long long)grid * 10;
+    long long it = block_size / (2 * warps);
+    return it < 1 ? 1 : (it > 8 ? 8 : (int)it);
+}
+
+static WaveArgs wave_args(pct_ctx* c, const WavePlan* pl, long long block_size, float lambda, float* x, float2* acc, WaveCtrl* ctrl, int grid) {
+    WaveArgs a{};
+    a.g = c->g;
+    a.H = pl ? offset_hist(c->H, pl->first) : c->H;
+    a.n = pl ? pl->n : c->n;
+    a.block_size = block_size;
+    a.n_blocks = pl ? pl->n_blocks : 1;
+    a.item = wave_item(block_size, grid);
+    a.n_slabs = c->shape.n_slabs;
+    a.n_sub = c->shape.n_sub;
+    a.slab_voxels = (long long)c->shape.slab_slices * c->g.nx * c->g.ny;
+    a.n_voxels = c->n_voxels;
+    a.lambda = lambda;
+    a.x = x;
+    a.acc = acc;
+    a.tab = c->tab;
+    a.ctrl = ctrl;
+    a.plan = pl ? pl->plan : nullptr;
+    a.need = pl ? pl->need : nullptr;
+    a.done = pl ? pl->done : nullptr;
+    return a;
+}
+
+// One DROP sweep over the histories of a plan, image x, accumulator acc (zero on entry and on exit), on stream s.
+// on_main: s is the context's stream and the histories may still be uploading (the launches then follow the upload
+// 64 blocks at a time).  launches (optional) counts the k_wave launches.
+static int wave_sweep(pct_ctx* c, WavePlan& pl, long long block_size, float lambda, float* x, float2* acc, WaveCtrl* ctrl, int grid,
+                      cudaStream_t s, bool on_main, int* launches = nullptr) {
+    // the sweep's queue, flags and counters start from zero (`error` is sticky, `last` holds the previous sweep's counters)
+    CUDA_TRY(c, cudaMemsetAsync(ctrl, 0, offsetof(WaveCtrl, error), s));
+    CUDA_TRY(c, cudaMemsetAsync(ctrl->cur, 0, sizeof(ctrl->cur), s));
+    CUDA_TRY(c, cudaMemsetAsync(ctrl->upd_seq, 0, 5 * sizeof(ctrl->upd_seq), s));
+    CUDA_TRY(c, cudaMemsetAsync(pl.done, 0, sizeof(int) * (size_t)pl.n_blocks * c->shape.n_slabs, s));
+    WaveArgs a = wave_args(c, &pl, block_size, lambda, x, acc, ctrl, grid);
+    for (long long q = 0; q < pl.n_blocks;) {
+        long long q1 = pl.n_blocks;
+        if (on_main) {
+            if (c->chunks_waited < c->chunk_ev.size() && q + kGraphPairs < q1) q1 = q + kGraphPairs;
+            if (int rc = wait_upload(c, q1 < pl.n_blocks ? pl.first + q1 * block_size : -1)) return rc;
+        }
+        if (int rc = build_plan(c, pl, block_size, q1, s)) return rc;
+        if (q > 0) CUDA_TRY(c, cudaMemsetAsync(&ctrl->ticket, 0, sizeof(ctrl->ticket), s));
+        a.q0 = q;
+        a.q1 = q1;
+        CUDA_TRY(c, launch_wave(a, grid, s));
+        if (launches) ++*launches;
+        q = q1;
+    }
+    CUDA_TRY(c, cudaMemcpyAsync(ctrl->last, ctrl->cur, sizeof(ctrl->cur), cudaMemcpyDeviceToDevice, s));
+    return PCT_OK;
+}
+
+// A wait that timed out or a row outside its planned slab range (both "cannot happen": DESIGN.md) is reported once.
+static int check_wave_error(pct_ctx* c) {
+    if (c->engine != 1) return PCT_OK;
+    unsigned err = 0;
+    CUDA_TRY(c, cudaMemcpyAsync(&err, &c->wctrl->error, sizeof(err), cudaMemcpyDeviceToHost, c->stream));
+    CUDA_TRY(c, cudaStreamSynchronize(c->stream));
+    for (int p = 0; p < c->carp_p && c->carp_wctrl; ++p) {
+        unsigned e = 0;
+        CUDA_TRY(c, cudaMemcpy(&e, &c->carp_wctrl[p].error, sizeof(e), cudaMemcpyDeviceToHost));
+        if (e) CUDA_TRY(c, cudaMemset(&c->carp_wctrl[p].error, 0, sizeof(e)));
+        err |= e;
+    }
+    if (!err) return PCT_OK;
+    CUDA_TRY(c, cudaMemsetAsync(&c->wctrl->error, 0, sizeof(err), c->stream));
+    return fail(c, PCT_EINTERNAL, "wavefront engine: %s; the image is not valid",
+                (err & 1u) ? "a path left the depth-slab range planned for it" : "a slab wait timed out");
+}
+
+static int iterate_wave(pct_ctx* c, float lambda, long long block_size, int n_iter) {
+    if (int rc = ensure_plans(c, block_size, 0)) return rc;
+    for (int it = 0; it < n_iter; ++it)
+        if (int rc = wave_sweep(c, c->plans[0], block_size, lambda, c->x, c->acc, c->wctrl, c->wave_grid, c->stream, true)) return rc;
+    return PCT_OK;
+}
+
 extern "C" int pct_iterate(pct_ctx* c, float lambda, int64_t block_size, int n_iter) {
     if (!c) return PCT_EINVAL;
     if (!c->have_hist) return fail(c, PCT_ESTATE, "pct_iterate: no histories set");
@@ -429,6 +649,8 @@ extern "C" int pct_iterate(pct_ctx* c, float lambda, int64_t block_size, int n_i
     if (block_size < 1 || block_size > (1LL << 24)) return fail(c, PCT_EINVAL, "pct_iterate: block_size must be in [1, 2^24]");
     if (n_iter < 0) return fail(c, PCT_EINVAL, "pct_iterate: n_iter must be >= 0");
     if (n_iter == 0) return PCT_OK;
+    DeviceGuard guard(c->device);
+    if (c->engine == 1) return iterate_wave(c, lambda, block_size, n_iter);
     const long long n_blocks = (c->n + block_size - 1) / block_size;
     const long long pairs = n_blocks * (long long)n_iter;
     CUDA_TRY(c, cudaMemsetAsync(c->ctrl, 0, sizeof(Ctrl), c->stream));
@@ -496,12 +718,18 @@ extern "C" int pct_iterate_carp(pct_ctx* c, float lambda, int64_t block_size, in
     if (int rc = wait_upload(c, -1)) return rc;
     const int P = n_strings;
     const long long M = c->n_voxels;
+    DeviceGuard guard(c->device);
+    // every string's image and accumulator start on a 16-byte boundary (the update reads them 128 bits at a time)
+    const long long stride = (M + 3) & ~3LL;
     if (c->carp_p != P) {
         release_carp(c);
-        CUDA_TRY(c, cudaMalloc(&c->carp_x, sizeof(float) * (size_t)M * P));
-        CUDA_TRY(c, cudaMalloc(&c->carp_acc, sizeof(float2) * (size_t)M * P));
+        c->carp_stride = stride;
+        CUDA_TRY(c, cudaMalloc(&c->carp_x, sizeof(float) * (size_t)stride * P));
+        CUDA_TRY(c, cudaMalloc(&c->carp_acc, sizeof(float2) * (size_t)stride * P));
         CUDA_TRY(c, cudaMalloc(&c->carp_ctrl, sizeof(Ctrl) * P));
-        CUDA_TRY(c, cudaMemsetAsync(c->carp_acc, 0, sizeof(float2) * (size_t)M * P, c->stream));
+        CUDA_TRY(c, cudaMalloc(&c->carp_wctrl, sizeof(WaveCtrl) * P));
+        CUDA_TRY(c, cudaMemsetAsync(c->carp_wctrl, 0, sizeof(WaveCtrl) * P, c->stream));
+        CUDA_TRY(c, cudaMemsetAsync(c->carp_acc, 0, sizeof(float2) * (size_t)stride * P, c->stream));
         CUDA_TRY(c, cudaEventCreateWithFlags(&c->carp_fork, cudaEventDisableTiming));
         for (int p = 0; p < P; ++p) {
             cudaStream_t s = nullptr;
@@ -513,8 +741,12 @@ extern "C" int pct_iterate_carp(pct_ctx* c, float lambda, int64_t block_size, in
         }
         c->carp_p = P;
     }
-    prepare_order(c, block_size, P);
-    if (c->order && c->order_built == 0) {  // every string's blocks, ordered by depth slab (k_order_blocks)
+    if (c->engine == 1) {
+        if (int rc = ensure_plans(c, block_size, P)) return rc;
+    } else {
+        prepare_order(c, block_size, P);
+    }
+    if (c->engine != 1 && c->order && c->order_built == 0) {  // every string's blocks, ordered by depth slab (k_order_blocks)
         for (int p = 0; p < P; ++p) {
             const long long lo = (long long)(((__int128)p * c->n) / P), hi = (long long)(((__int128)(p + 1) * c->n) / P);
             HistPtrs Hs = c->H;
@@ -529,9 +761,18 @@ extern "C" int pct_iterate_carp(pct_ctx* c, float lambda, int64_t block_size, in
         for (int p = 0; p < P; ++p) {
             cudaStream_t s = c->carp_stream[p];
             const long long lo = (long long)(((__int128)p * c->n) / P), hi = (long long)(((__int128)(p + 1) * c->n) / P);
-            float* xs = c->carp_x + (size_t)p * M;
+            float* xs = c->carp_x + (size_t)p * stride;
             CUDA_TRY(c, cudaStreamWaitEvent(s, c->carp_fork, 0));
             CUDA_TRY(c, cudaMemcpyAsync(xs, c->x, sizeof(float) * M, cudaMemcpyDeviceToDevice, s));  // the common x0
+            if (c->engine == 1) {
+                // every string gets its share of the CTA slots: P persistent launches side by side
+                const int grid_p = (c->wave_grid + P - 1) / P;
+                if (int rc = wave_sweep(c, c->plans[p], block_size, lambda, xs, c->carp_acc + (size_t)p * stride, c->carp_wctrl + p, grid_p, s, false))
+                    return rc;
+                CUDA_TRY(c, cudaEventRecord(c->carp_done[p], s));
+                CUDA_TRY(c, cudaStreamWaitEvent(c->stream, c->carp_done[p], 0));
+                continue;
+            }
             CUDA_TRY(c, cudaMemsetAsync(c->carp_ctrl + p, 0, sizeof(Ctrl), s));
             DropArgs a = drop_args(c, block_size, -1, 0);
             a.H.t_in += lo; a.H.v_in += lo; a.H.t_out += lo; a.H.v_out += lo;
@@ -539,7 +780,7 @@ extern "C" int pct_iterate_carp(pct_ctx* c, float lambda, int64_t block_size, in
             a.H.wepl += lo; a.H.proj += lo;
             a.n = hi - lo;
             a.x = xs;
-            a.acc = c->carp_acc + (size_t)p * M;
+            a.acc = c->carp_acc + (size_t)p * stride;
             a.ctrl = c->carp_ctrl + p;
             a.order = c->order ? c->order + lo : nullptr;
             const long long n_blocks = (a.n + block_size - 1) / block_size;
@@ -553,7 +794,9 @@ extern "C" int pct_iterate_carp(pct_ctx* c, float lambda, int64_t block_size, in
             CUDA_TRY(c, cudaEventRecord(c->carp_done[p], s));
             CUDA_TRY(c, cudaStreamWaitEvent(c->stream, c->carp_done[p], 0));
         }
-        CUDA_TRY(c, launch_mean(c->x, c->carp_x, P, M, c->stream));
+        CUDA_TRY(c, launch_mean(c->x, c->carp_x, P, M, stride, c->stream));
+        if (c->engine == 1)  // pct_get_stats: the counters of the strings' sweeps, added up
+            CUDA_TRY(c, launch_sum_stats(c->wctrl, c->carp_wctrl, P, c->stream));
     }
     return PCT_OK;
 }
@@ -570,23 +813,26 @@ extern "C" int pct_set_path_model(pct_ctx* c, int model) {
 
 extern "C" int pct_synchronize(pct_ctx* c) {
     if (!c) return PCT_EINVAL;
+    DeviceGuard guard(c->device);
     if (int rc = wait_upload(c, -1)) return rc;  // the host arrays are free once this returns
     CUDA_TRY(c, cudaStreamSynchronize(c->stream));
-    return PCT_OK;
+    return check_wave_error(c);
 }
 
 extern "C" int pct_get_image(pct_ctx* c, float* dst, int64_t n_voxels) {
     if (!c) return PCT_EINVAL;
     if (!dst || n_voxels != c->n_voxels) return fail(c, PCT_EINVAL, "pct_get_image: dst NULL or n_voxels != nx*ny*nz");
+    DeviceGuard guard(c->device);
     if (int rc = wait_upload(c, -1)) return rc;
     CUDA_TRY(c, cudaMemcpyAsync(dst, c->x, sizeof(float) * c->n_voxels, cudaMemcpyDefault, c->stream));
     CUDA_TRY(c, cudaStreamSynchronize(c->stream));
-    return PCT_OK;
+    return check_wave_error(c);
 }
 
 extern "C" int pct_set_image(pct_ctx* c, const float* src, int64_t n_voxels) {
     if (!c) return PCT_EINVAL;
     if (!src || n_voxels != c->n_voxels) return fail(c, PCT_EINVAL, "pct_set_image: src NULL or n_voxels != nx*ny*nz");
+    DeviceGuard guard(c->device);
     CUDA_TRY(c, cudaMemcpyAsync(c->x, src, sizeof(float) * c->n_voxels, cudaMemcpyDefault, c->stream));
     if (!is_device_ptr(src)) CUDA_TRY(c, cudaStreamSynchronize(c->stream));
     return PCT_OK;
@@ -594,12 +840,14 @@ extern "C" int pct_set_image(pct_ctx* c, const float* src, int64_t n_voxels) {
 
 extern "C" int pct_get_stats(pct_ctx* c, int64_t out[4]) {
     if (!c || !out) return PCT_EINVAL;
-    Ctrl h;
-    CUDA_TRY(c, cudaMemcpyAsync(&h, c->ctrl, sizeof(Ctrl), cudaMemcpyDeviceToHost, c->stream));
+    DeviceGuard guard(c->device);
+    unsigned long long last[4] = {0, 0, 0, 0};
+    const void* src = c->engine == 1 ? (const void*)c->wctrl->last : (const void*)c->ctrl->last;
+    CUDA_TRY(c, cudaMemcpyAsync(last, src, sizeof(last), cudaMemcpyDeviceToHost, c->stream));
     CUDA_TRY(c, cudaStreamSynchronize(c->stream));
-    for (int i = 0; i < 3; ++i) out[i] = (int64_t)h.last[i];
+    for (int i = 0; i < 3; ++i) out[i] = (int64_t)last[i];
     out[3] = c->n;
-    return PCT_OK;
+    return check_wave_error(c);
 }
 
 extern "C" int pct_debug_rows(pct_ctx* c, int64_t first, int64_t count, int32_t max_seg, int32_t* nseg, int32_t* nnz,
@@ -621,6 +869,7 @@ extern "C" int pct_debug_rows(pct_ctx* c, int64_t first, int64_t count, int32_t 
     a.tab = c->tab;
     a.nseg = nseg; a.nnz = nnz; a.seg_idx = seg_idx;
     a.seg_len = seg_len; a.row_len = row_len; a.nodes = nodes;
+    DeviceGuard guard(c->device);
     if (int rc = wait_upload(c, first + count)) return rc;
     CUDA_TRY(c, launch_rows(a, c->stream));
     return PCT_OK;
@@ -632,7 +881,19 @@ extern "C" int pct_debug_block(pct_ctx* c, int64_t first, int64_t count, float* 
     if (first < 0 || count < 1 || first + count > c->n) return fail(c, PCT_EINVAL, "pct_debug_block: range outside the histories");
     if (!delta || !cnt || !is_device_ptr(delta) || !is_device_ptr(cnt))
         return fail(c, PCT_EINVAL, "pct_debug_block: delta and cnt must be device memory");
+    if (count > (1LL << 24)) return fail(c, PCT_EINVAL, "pct_debug_block: count must be <= 2^24 (hit counts are held exactly in fp32)");
+    DeviceGuard guard(c->device);
     if (int rc = wait_upload(c, first + count)) return rc;
+    if (c->engine == 1) {  // the wavefront kernel in its plain mode: the range as ONE block in the caller's order, no update
+        CUDA_TRY(c, cudaMemsetAsync(&c->wctrl->ticket, 0, sizeof(c->wctrl->ticket), c->stream));
+        WaveArgs w = wave_args(c, nullptr, count, 1.0f, c->x, c->acc, c->wctrl, c->wave_grid);
+        w.first = first;
+        w.count = count;
+        CUDA_TRY(c, launch_wave(w, c->wave_grid, c->stream));
+        CUDA_TRY(c, launch_split_acc(c->acc, delta, cnt, c->n_voxels, c->stream));
+        CUDA_TRY(c, cudaMemsetAsync(c->wctrl->cur, 0, sizeof(c->wctrl->cur), c->stream));
+        return PCT_OK;
+    }
     CUDA_TRY(c, cudaMemsetAsync(c->ctrl, 0, sizeof(Ctrl), c->stream));
     const DropArgs a = drop_args(c, count, first, count);
     CUDA_TRY(c, launch_drop_block(a, c->drop_grid, c->stream));
@@ -647,8 +908,32 @@ extern "C" int pct_profile_sweep(pct_ctx* c, float lambda, int64_t block_size, f
     if (!c->have_hist) return fail(c, PCT_ESTATE, "pct_profile_sweep: no histories set");
     if (!(lambda > 0.0f) || !(lambda < 2.0f)) return fail(c, PCT_EINVAL, "pct_profile_sweep: lambda must be in (0, 2)");
     if (block_size < 1 || block_size > (1LL << 24)) return fail(c, PCT_EINVAL, "pct_profile_sweep: block_size must be in [1, 2^24]");
+    DeviceGuard guard(c->device);
     if (int rc = wait_upload(c, -1)) return rc;
     const long long n_blocks = (c->n + block_size - 1) / block_size;
+    if (c->engine == 1) {  // one persistent launch per sweep: its device time IS the sweep's
+        if (int rc = ensure_plans(c, block_size, 0)) return rc;
+        if (int rc = build_plan(c, c->plans[0], block_size, n_blocks, c->stream)) return rc;  // (the plan is made once per history set: not timed)
+        cudaEvent_t e0 = nullptr, e1 = nullptr;
+        CUDA_TRY(c, cudaEventCreate(&e0));
+        cudaError_t e = cudaEventCreate(&e1);
+        int launches = 0, rc = PCT_OK;
+        float ms = 0.f;
+        if (e == cudaSuccess) e = cudaEventRecord(e0, c->stream);
+        if (e == cudaSuccess) rc = wave_sweep(c, c->plans[0], block_size, lambda, c->x, c->acc, c->wctrl, c->wave_grid, c->stream, true, &launches);
+        if (e == cudaSuccess && rc == PCT_OK) e = cudaEventRecord(e1, c->stream);
+        if (e == cudaSuccess && rc == PCT_OK) e = cudaStreamSynchronize(c->stream);
+        if (e == cudaSuccess && rc == PCT_OK) e = cudaEventElapsedTime(&ms, e0, e1);
+        cudaEventDestroy(e0);
+        if (e1) cudaEventDestroy(e1);
+        if (rc != PCT_OK) return rc;
+        CUDA_TRY(c, e);
+        out_ms[0] = ms;
+        out_ms[1] = 0.f;
+        out_ms[2] = ms;
+        out_ms[3] = (float)launches;
+        return check_wave_error(c);
+    }
     const int kChunk = 256;  // blocks per batch of events
     cudaEvent_t ev[2 * kChunk + 1];
     int made = 0;

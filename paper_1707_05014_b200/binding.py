@@ -176,9 +176,10 @@ def pct_profile_sweep(ctx, lam, block_size):
 
 def pct_measure_peaks(footprint_bytes, cuda_stream=None):
     """Micro-benchmarks behind the roofline (include/pct.h: pct_measure_peaks) -> dict."""
-    out = (C.c_double * 8)()
+    out = (C.c_double * 12)()
     rc = lib().pct_measure_peaks(cuda_stream, int(footprint_bytes), out)
     if rc != PCT_OK:
         raise PctError(rc, "pct_measure_peaks failed")
     return dict(gather_random_per_s=out[0], gather_path_per_s=out[1], red_v2_random_per_s=out[2], stream_read_bytes_per_s=out[3],
-                ffma_inst_per_s=out[4], ffma2_inst_per_s=out[5], red_v2_path_per_s=out[6], footprint_bytes=int(out[7]))
+                ffma_inst_per_s=out[4], ffma2_inst_per_s=out[5], red_v2_path_per_s=out[6], footprint_bytes=int(out[7]),
+                gather_path_tiled_per_s=out[8], red_v2_path_tiled_per_s=out[9])

@@ -30,7 +30,9 @@ struct pct_ctx {
     int device = 0;
     cudaStream_t stream = nullptr;
     Geom g{};
-    long long n_voxels = 0;
+    long long n_voxels = 0;  // nx*ny*nz: the caller's image
+    long long n_slots = 0;   // voxels as stored (slices of nxp x nyp, voxel_slot): what the kernels work on
+    float* io_buf = nullptr; // n_voxels floats: the image in the caller's order on its way in or out
     float* x = nullptr;
     float2* acc = nullptr;
     float4* tab = nullptr;
@@ -67,8 +69,9 @@ struct pct_ctx {
     std::vector<cudaStream_t> carp_stream;
     std::vector<cudaEvent_t> carp_done;
     cudaEvent_t carp_fork = nullptr;
-    // wavefront engine (pct_wave.cu): the default; PCT_ENGINE=blocks selects the launch-pair-per-block engine
-    int engine = 1;
+    // 0: the block engine (two launches per DROP block, replayed from a CUDA graph): the default, the faster one at
+    // every config measured; 1: the wavefront engine (pct_wave.cu, one persistent launch per sweep), PCT_ENGINE=wave
+    int engine = 0;
     int sm_count = 148;
     int wave_grid = 0;
     WaveShape shape{};
@@ -190,7 +193,7 @@ static void prepare_order(pct_ctx* c, long long block_size, int strings = 0) {
     int mode = PCT_ORDER_BLOCKS;
     if (const char* env = getenv("PCT_ORDER"))  // tuning / test override: 0 never, 1 by footprint, 2 always
         if (env[0] >= '0' && env[0] <= '2' && env[1] == 0) mode = env[0] - '0';
-    const bool wanted = mode == 2 || (mode == 1 && 12.0 * images * (double)c->n_voxels > 0.85 * l2);
+    const bool wanted = mode == 2 || (mode == 1 && 12.0 * images * (double)c->n_slots > 0.85 * l2);
     if (!wanted || block_size < 1024) {  // (small blocks: nothing to gain)
         if (c->order) cudaFree(c->order);
         c->order = nullptr;
@@ -198,7 +201,7 @@ static void prepare_order(pct_ctx* c, long long block_size, int strings = 0) {
         return;
     }
     const double per_slab = 0.25 * l2;
-    const double want = ceil(12.0 * images * (double)c->n_voxels / per_slab);
+    const double want = ceil(12.0 * images * (double)c->n_slots / per_slab);
     c->order_slabs = want < 4.0 ? 4 : (want > 64.0 ? 64 : (int)want);
     if (c->order && c->order_block == block_size && c->order_strings == strings) return;
     if (!c->order && cudaMalloc(&c->order, sizeof(uint32_t) * (size_t)c->n) != cudaSuccess) {
@@ -283,6 +286,13 @@ extern "C" int pct_create(pct_ctx** out, int nx, int ny, int nz, float h, float 
     if (!c) return fail(nullptr, PCT_ENOMEM, "pct_create: out of host memory");
     c->g = g;
     c->n_voxels = (long long)nx * ny * nz;
+    c->g.nxp = (nx + 1) & ~1;
+    c->g.slice_p = c->g.nxp * ((ny + 1) & ~1);
+    c->n_slots = (long long)c->g.slice_p * nz;
+    if (c->n_slots >= (1LL << 31)) {
+        delete c;
+        return fail(nullptr, PCT_EINVAL, "pct_create: the stored image (nx, ny rounded up to even) must have < 2^31 voxels");
+    }
     c->stream = (cudaStream_t)stream;
     int rc = PCT_OK;
     auto body = [&]() -> int {
@@ -290,12 +300,13 @@ extern "C" int pct_create(pct_ctx** out, int nx, int ny, int nz, float h, float 
         int l2 = 0;
         CUDA_TRY(nullptr, cudaDeviceGetAttribute(&l2, cudaDevAttrL2CacheSize, c->device));
         c->l2_bytes = (double)l2;
-        CUDA_TRY(nullptr, cudaMalloc(&c->x, sizeof(float) * c->n_voxels));
-        CUDA_TRY(nullptr, cudaMalloc(&c->acc, sizeof(float2) * c->n_voxels));
+        CUDA_TRY(nullptr, cudaMalloc(&c->x, sizeof(float) * c->n_slots));
+        CUDA_TRY(nullptr, cudaMalloc(&c->acc, sizeof(float2) * c->n_slots));
+        CUDA_TRY(nullptr, cudaMalloc(&c->io_buf, sizeof(float) * c->n_voxels));
         CUDA_TRY(nullptr, cudaMalloc(&c->tab, sizeof(float4) * (nmin + 1)));
         CUDA_TRY(nullptr, cudaMalloc(&c->ctrl, sizeof(Ctrl)));
-        CUDA_TRY(nullptr, cudaMemsetAsync(c->x, 0, sizeof(float) * c->n_voxels, c->stream));
-        CUDA_TRY(nullptr, cudaMemsetAsync(c->acc, 0, sizeof(float2) * c->n_voxels, c->stream));
+        CUDA_TRY(nullptr, cudaMemsetAsync(c->x, 0, sizeof(float) * c->n_slots, c->stream));
+        CUDA_TRY(nullptr, cudaMemsetAsync(c->acc, 0, sizeof(float2) * c->n_slots, c->stream));
         CUDA_TRY(nullptr, cudaMemsetAsync(c->ctrl, 0, sizeof(Ctrl), c->stream));
         float4* tab = (float4*)malloc(sizeof(float4) * (nmin + 1));
         if (!tab) return fail(nullptr, PCT_ENOMEM, "pct_create: out of host memory");
@@ -307,14 +318,14 @@ extern "C" int pct_create(pct_ctx** out, int nx, int ny, int nz, float h, float 
         CUDA_TRY(nullptr, cudaDeviceGetAttribute(&c->sm_count, cudaDevAttrMultiProcessorCount, c->device));
         CUDA_TRY(nullptr, cudaMalloc(&c->wctrl, sizeof(WaveCtrl)));
         CUDA_TRY(nullptr, cudaMemsetAsync(c->wctrl, 0, sizeof(WaveCtrl), c->stream));
-        c->shape = wave_shape(g);
-        if (const char* env = getenv("PCT_ENGINE")) c->engine = strcmp(env, "blocks") == 0 ? 0 : 1;
+        c->shape = wave_shape(c->g);
+        if (const char* env = getenv("PCT_ENGINE")) c->engine = strcmp(env, "wave") == 0 ? 1 : 0;
         // the per-warp row buffer and the two staged copies of the table must fit the shared memory of an SM
         int smem_max = 0;
         CUDA_TRY(nullptr, cudaDeviceGetAttribute(&smem_max, cudaDevAttrMaxSharedMemoryPerBlockOptin, c->device));
-        if (drop_smem_bytes(nmin) > (size_t)smem_max) {
+        if (wave_smem_need(nmin) > (size_t)smem_max) {
             snprintf(g_create_err, 512, "pct_create: min(nx,ny) = %d needs %zu B of shared memory per CTA, the device offers %d",
-                     nmin, drop_smem_bytes(nmin), smem_max);
+                     nmin, wave_smem_need(nmin), smem_max);
             return PCT_EINVAL;
         }
         CUDA_TRY(nullptr, drop_configure(nmin, &c->drop_grid));
@@ -361,6 +372,7 @@ extern "C" void pct_destroy(pct_ctx* c) {
     release_histories(c);
     if (c->copy_stream) cudaStreamDestroy(c->copy_stream);
     if (c->x) cudaFree(c->x);
+    if (c->io_buf) cudaFree(c->io_buf);
     if (c->acc) cudaFree(c->acc);
     if (c->tab) cudaFree(c->tab);
     if (c->ctrl) cudaFree(c->ctrl);
@@ -501,7 +513,7 @@ static DropArgs drop_args(pct_ctx* c, long long block_size, long long first, lon
 
 static int enqueue_pair(pct_ctx* c, const DropArgs& a, float lambda, long long n_blocks, cudaStream_t s) {
     CUDA_TRY(c, launch_drop_block(a, c->drop_grid, s));
-    CUDA_TRY(c, launch_update(c->x, c->acc, c->n_voxels, lambda, c->ctrl, n_blocks, s));
+    CUDA_TRY(c, launch_update(c->x, c->acc, c->n_slots, lambda, c->ctrl, n_blocks, s));
     return PCT_OK;
 }
 
@@ -560,7 +572,7 @@ static int wave_item(long long block_size, int grid) {
         const int v = atoi(env);
         if (v >= 1 && v <= 16) return v;
     }
-    const long long warps = (long long)grid * 10;
+    const long long warps = (long long)grid * wave_walkers_per_cta();
     long long it = block_size / (2 * warps);
     return it < 1 ? 1 : (it > 8 ? 8 : (int)it);
 }
@@ -575,8 +587,8 @@ static WaveArgs wave_args(pct_ctx* c, const WavePlan* pl, long long block_size, 
     a.item = wave_item(block_size, grid);
     a.n_slabs = c->shape.n_slabs;
     a.n_sub = c->shape.n_sub;
-    a.slab_voxels = (long long)c->shape.slab_slices * c->g.nx * c->g.ny;
-    a.n_voxels = c->n_voxels;
+    a.slab_voxels = (long long)c->shape.slab_slices * c->g.slice_p;
+    a.n_voxels = c->n_slots;
     a.lambda = lambda;
     a.x = x;
     a.acc = acc;
@@ -717,7 +729,7 @@ extern "C" int pct_iterate_carp(pct_ctx* c, float lambda, int64_t block_size, in
     if (n_iter == 0) return PCT_OK;
     if (int rc = wait_upload(c, -1)) return rc;
     const int P = n_strings;
-    const long long M = c->n_voxels;
+    const long long M = c->n_slots;  // (the strings' images live in storage order like the context's)
     DeviceGuard guard(c->device);
     // every string's image and accumulator start on a 16-byte boundary (the update reads them 128 bits at a time)
     const long long stride = (M + 3) & ~3LL;
@@ -824,7 +836,10 @@ extern "C" int pct_get_image(pct_ctx* c, float* dst, int64_t n_voxels) {
     if (!dst || n_voxels != c->n_voxels) return fail(c, PCT_EINVAL, "pct_get_image: dst NULL or n_voxels != nx*ny*nz");
     DeviceGuard guard(c->device);
     if (int rc = wait_upload(c, -1)) return rc;
-    CUDA_TRY(c, cudaMemcpyAsync(dst, c->x, sizeof(float) * c->n_voxels, cudaMemcpyDefault, c->stream));
+    // storage order -> the caller's order, straight into dst if it is device memory
+    float* out = is_device_ptr(dst) ? dst : c->io_buf;
+    CUDA_TRY(c, launch_image_io(c->x, out, c->g, false, c->stream));
+    if (out != dst) CUDA_TRY(c, cudaMemcpyAsync(dst, out, sizeof(float) * c->n_voxels, cudaMemcpyDeviceToHost, c->stream));
     CUDA_TRY(c, cudaStreamSynchronize(c->stream));
     return check_wave_error(c);
 }
@@ -833,8 +848,10 @@ extern "C" int pct_set_image(pct_ctx* c, const float* src, int64_t n_voxels) {
     if (!c) return PCT_EINVAL;
     if (!src || n_voxels != c->n_voxels) return fail(c, PCT_EINVAL, "pct_set_image: src NULL or n_voxels != nx*ny*nz");
     DeviceGuard guard(c->device);
-    CUDA_TRY(c, cudaMemcpyAsync(c->x, src, sizeof(float) * c->n_voxels, cudaMemcpyDefault, c->stream));
-    if (!is_device_ptr(src)) CUDA_TRY(c, cudaStreamSynchronize(c->stream));
+    const bool dev = is_device_ptr(src);
+    if (!dev) CUDA_TRY(c, cudaMemcpyAsync(c->io_buf, src, sizeof(float) * c->n_voxels, cudaMemcpyHostToDevice, c->stream));
+    CUDA_TRY(c, launch_image_io(c->x, dev ? const_cast<float*>(src) : c->io_buf, c->g, true, c->stream));
+    if (!dev) CUDA_TRY(c, cudaStreamSynchronize(c->stream));
     return PCT_OK;
 }
 
@@ -847,6 +864,7 @@ extern "C" int pct_get_stats(pct_ctx* c, int64_t out[4]) {
     CUDA_TRY(c, cudaStreamSynchronize(c->stream));
     for (int i = 0; i < 3; ++i) out[i] = (int64_t)last[i];
     out[3] = c->n;
+    wave_prof_dump("pct_get_stats");
     return check_wave_error(c);
 }
 
@@ -890,14 +908,14 @@ extern "C" int pct_debug_block(pct_ctx* c, int64_t first, int64_t count, float* 
         w.first = first;
         w.count = count;
         CUDA_TRY(c, launch_wave(w, c->wave_grid, c->stream));
-        CUDA_TRY(c, launch_split_acc(c->acc, delta, cnt, c->n_voxels, c->stream));
+        CUDA_TRY(c, launch_split_acc(c->acc, delta, cnt, c->g, c->stream));
         CUDA_TRY(c, cudaMemsetAsync(c->wctrl->cur, 0, sizeof(c->wctrl->cur), c->stream));
         return PCT_OK;
     }
     CUDA_TRY(c, cudaMemsetAsync(c->ctrl, 0, sizeof(Ctrl), c->stream));
     const DropArgs a = drop_args(c, count, first, count);
     CUDA_TRY(c, launch_drop_block(a, c->drop_grid, c->stream));
-    CUDA_TRY(c, launch_split_acc(c->acc, delta, cnt, c->n_voxels, c->stream));
+    CUDA_TRY(c, launch_split_acc(c->acc, delta, cnt, c->g, c->stream));
     CUDA_TRY(c, cudaMemsetAsync(c->ctrl, 0, sizeof(Ctrl), c->stream));
     return PCT_OK;
 }
@@ -951,7 +969,7 @@ extern "C" int pct_profile_sweep(pct_ctx* c, float lambda, int64_t block_size, f
             for (int i = 0; i < nb; ++i) {
                 CUDA_TRY(c, launch_drop_block(a, c->drop_grid, c->stream));
                 CUDA_TRY(c, cudaEventRecord(ev[2 * i + 1], c->stream));
-                CUDA_TRY(c, launch_update(c->x, c->acc, c->n_voxels, lambda, c->ctrl, n_blocks, c->stream));
+                CUDA_TRY(c, launch_update(c->x, c->acc, c->n_slots, lambda, c->ctrl, n_blocks, c->stream));
                 CUDA_TRY(c, cudaEventRecord(ev[2 * i + 2], c->stream));
             }
             CUDA_TRY(c, cudaStreamSynchronize(c->stream));

@@ -56,7 +56,8 @@ cudaError_t drop_configure(int nmin, int* grid_out);
 cudaError_t launch_drop_block(const DropArgs& a, int grid, cudaStream_t stream);
 cudaError_t launch_update(float* x, float2* acc, long long n_voxels, float lambda, Ctrl* ctrl,
                           long long n_blocks, cudaStream_t stream);
-cudaError_t launch_split_acc(float2* acc, float* delta, float* cnt, long long n_voxels, cudaStream_t stream);
+cudaError_t launch_split_acc(float2* acc, float* delta, float* cnt, const Geom& g, cudaStream_t stream);
+cudaError_t launch_image_io(float* x, float* ext, const Geom& g, bool to_storage, cudaStream_t stream);
 cudaError_t launch_rows(const RowsArgs& a, cudaStream_t stream);
 cudaError_t launch_mean(float* x, const float* xs, int n_strings, long long n_voxels, long long pitch, cudaStream_t stream);
 cudaError_t launch_order_blocks(const HistPtrs& H, const Geom& g, long long n, long long block_size, long long first_block,
@@ -73,17 +74,16 @@ constexpr int kMaxSlabs = 32;
 
 struct alignas(128) WaveCtrl {
     unsigned long long ticket;    // next work item of the launch
-    int pending;                  // update sub-tasks posted and not yet claimed (a hint: warps look for one only when > 0)
+    unsigned int unused;
     unsigned int error;           // sticky: 1 = a row left the slab range its plan declared, 2 = a wait timed out
     unsigned long long cur[4];    // running counters of the current sweep: rows, nnz, segments, -
     unsigned long long last[4];   // counters of the last completed sweep
     unsigned int pad[12];
-    // one 128 B line each (all indexed by slab)
+    // indexed by slab, one or two 128 B lines each
     unsigned int upd_seq[kMaxSlabs];   // the slab holds the image after blocks [0, upd_seq) of the sweep
     unsigned int post_seq[kMaxSlabs];  // block whose update was posted last
-    unsigned int posted[kMaxSlabs];    // updates posted so far (sweep)
-    unsigned int claimed[kMaxSlabs];   // update sub-tasks claimed so far
-    unsigned int finished[kMaxSlabs];  // update sub-tasks finished so far
+    unsigned int finished[kMaxSlabs];  // update sub-tasks finished so far (sweep)
+    unsigned long long tasks[kMaxSlabs];  // low half: update sub-tasks posted so far (sweep), high half: claimed so far
 };
 static_assert(sizeof(WaveCtrl) == 128 * 6, "WaveCtrl layout");
 
@@ -113,7 +113,10 @@ struct WaveShape {
     int n_slabs, slab_slices, n_sub;
 };
 WaveShape wave_shape(const Geom& g);
+int wave_walkers_per_cta();
+size_t wave_smem_need(int nmin);
 cudaError_t wave_configure(int nmin, int* grid_out);
+void wave_prof_dump(const char* tag);  // (a no-op unless built with -DPCT_WAVE_PROF)
 cudaError_t launch_sum_stats(WaveCtrl* dst, const WaveCtrl* strings, int n_strings, cudaStream_t stream);
 cudaError_t launch_wave(const WaveArgs& a, int grid, cudaStream_t stream);
 cudaError_t launch_plan_blocks(const HistPtrs& H, const Geom& g, long long n, long long block_size, long long first_block,

@@ -312,22 +312,49 @@ cudaError_t launch_update(float* x, float2* acc, long long n_voxels, float lambd
     return cudaGetLastError();
 }
 
-// inspection: de-interleave the accumulator into Delta and c, and zero it
-__global__ void k_split_acc(float2* __restrict__ acc, float* __restrict__ delta, float* __restrict__ cnt, long long n) {
+// inspection: de-interleave the accumulator into Delta and c (in the voxel order of include/pct.h), and zero it
+__global__ void k_split_acc(float2* __restrict__ acc, float* __restrict__ delta, float* __restrict__ cnt, Geom g) {
+    const long long n = (long long)g.nx * g.ny * g.nz;
     const long long stride = (long long)gridDim.x * blockDim.x;
-    for (long long j = (long long)blockIdx.x * blockDim.x + threadIdx.x; j < n; j += stride) {
-        const float2 dc = acc[j];
-        delta[j] = dc.x;
-        cnt[j] = dc.y;
-        acc[j] = make_float2(0.f, 0.f);
+    for (long long v = (long long)blockIdx.x * blockDim.x + threadIdx.x; v < n; v += stride) {
+        const int i = (int)(v % g.nx), j = (int)((v / g.nx) % g.ny), k = (int)(v / ((long long)g.nx * g.ny));
+        const int slot = voxel_slot(i, j, k, g.nxp, g.slice_p);
+        const float2 dc = acc[slot];
+        delta[v] = dc.x;
+        cnt[v] = dc.y;
+        acc[slot] = make_float2(0.f, 0.f);
     }
 }
 
-cudaError_t launch_split_acc(float2* acc, float* delta, float* cnt, long long n, cudaStream_t stream) {
+cudaError_t launch_split_acc(float2* acc, float* delta, float* cnt, const Geom& g, cudaStream_t stream) {
+    const long long n = (long long)g.nx * g.ny * g.nz;
     long long blocks = (n + 255) / 256;
     const long long cap = (long long)sm_count() * 16;
     if (blocks > cap) blocks = cap;
-    k_split_acc<<<(int)blocks, 256, 0, stream>>>(acc, delta, cnt, n);
+    k_split_acc<<<(int)blocks, 256, 0, stream>>>(acc, delta, cnt, g);
+    return cudaGetLastError();
+}
+
+// Image I/O: the caller's order i + nx (j + ny k) <-> the storage order (voxel_slot).  to_storage: ext -> x, else x -> ext.
+__global__ void k_image_io(float* __restrict__ x, float* __restrict__ ext, Geom g, bool to_storage) {
+    const long long n = (long long)g.nx * g.ny * g.nz;
+    const long long stride = (long long)gridDim.x * blockDim.x;
+    for (long long v = (long long)blockIdx.x * blockDim.x + threadIdx.x; v < n; v += stride) {
+        const int i = (int)(v % g.nx), j = (int)((v / g.nx) % g.ny), k = (int)(v / ((long long)g.nx * g.ny));
+        const int slot = voxel_slot(i, j, k, g.nxp, g.slice_p);
+        if (to_storage)
+            x[slot] = ext[v];
+        else
+            ext[v] = x[slot];
+    }
+}
+
+cudaError_t launch_image_io(float* x, float* ext, const Geom& g, bool to_storage, cudaStream_t stream) {
+    const long long n = (long long)g.nx * g.ny * g.nz;
+    long long blocks = (n + 255) / 256;
+    const long long cap = (long long)sm_count() * 16;
+    if (blocks > cap) blocks = cap;
+    k_image_io<<<(int)blocks, 256, 0, stream>>>(x, ext, g, to_storage);
     return cudaGetLastError();
 }
 
@@ -367,7 +394,15 @@ __global__ void __launch_bounds__(kThreads) k_rows(const RowsArgs a) {
             // the row as the hot path sees it: read back from the row buffer, segment-major
             for (int k = lane; k <= K; k += 32) {
                 const float2 e = row[row_slot(k)];
-                if (em.seg_idx) em.seg_idx[k] = __float_as_int(e.x);
+                if (em.seg_idx) {  // reported as the linear index i + nx (j + ny k) of include/pct.h, not as the storage slot
+                    int lin = __float_as_int(e.x);
+                    if (lin >= 0) {
+                        int vi, vj, vk;
+                        voxel_of_slot(lin, g.nxp, g.slice_p, vi, vj, vk);
+                        lin = vi + g.nx * (vj + g.ny * vk);
+                    }
+                    em.seg_idx[k] = lin;
+                }
                 if (em.seg_len && __float_as_int(e.x) >= 0) em.seg_len[k] = fabsf(e.y);
                 if (em.row_len) em.row_len[k] = __float_as_int(e.y) < 0 ? 1.0f : 0.0f;
             }

@@ -47,6 +47,7 @@ __global__ void __launch_bounds__(256) k_gather_random(const float* __restrict__
 // The path's access shape: the 32 lanes of a request touch 32 voxels one voxel apart along a random in-plane
 // direction of a volume nx x nx x nz words (nx a power of two), as the segment-major passes of the row projection
 // do: neighbouring lanes share a 32 B sector when the direction is close to the x axis.
+template <bool TILED>
 __device__ __forceinline__ uint32_t path_index(uint32_t& s, int lane, int nx, int nz) {
     const uint32_t r0 = next_rand(s), r1 = next_rand(s);
     const float ax = (float)(r0 & 63u) - 31.5f, ay = (float)((r0 >> 6) & 63u) - 31.5f;
@@ -54,9 +55,13 @@ __device__ __forceinline__ uint32_t path_index(uint32_t& s, int lane, int nx, in
     const int xi = ((int)(r0 >> 12) + __float2int_rn(ax * inv)) & (nx - 1);
     const int yi = ((int)(r1 & 0xffffu) + __float2int_rn(ay * inv)) & (nx - 1);
     const uint32_t z = (uint32_t)(((uint64_t)(r1 >> 16) * (uint32_t)nz) >> 16);
+    if (TILED)  // 2 x 2 in-plane tiles, two x-adjacent tiles side by side: a 32 B sector = 4 x 2 words or 2 x 2 pairs
+        return z * (uint32_t)nx * (uint32_t)nx + ((((uint32_t)yi >> 1) * ((uint32_t)nx >> 1) + ((uint32_t)xi >> 1)) << 2) +
+               (((uint32_t)yi & 1u) << 1) + ((uint32_t)xi & 1u);
     return (z * (uint32_t)nx + (uint32_t)yi) * (uint32_t)nx + (uint32_t)xi;
 }
 
+template <bool TILED>
 __global__ void __launch_bounds__(256) k_gather_paths(const float* __restrict__ buf, int nx, int nz, int iters, float* sink) {
     const int lane = threadIdx.x & 31;
     uint32_t s = seed_of((blockIdx.x * blockDim.x + threadIdx.x) >> 5);  // warp-uniform stream
@@ -64,20 +69,21 @@ __global__ void __launch_bounds__(256) k_gather_paths(const float* __restrict__ 
     for (int it = 0; it < iters; ++it) {
         float v[kIlp];
 #pragma unroll
-        for (int u = 0; u < kIlp; ++u) v[u] = __ldcg(buf + path_index(s, lane, nx, nz));
+        for (int u = 0; u < kIlp; ++u) v[u] = __ldcg(buf + path_index<TILED>(s, lane, nx, nz));
 #pragma unroll
         for (int u = 0; u < kIlp; ++u) acc += v[u];
     }
     if (acc == 123.456f) *sink = acc;
 }
 
+template <bool TILED>
 __global__ void __launch_bounds__(256) k_red_paths(float2* __restrict__ buf, int nx, int nz, int iters) {
     const int lane = threadIdx.x & 31;
     uint32_t s = seed_of((blockIdx.x * blockDim.x + threadIdx.x) >> 5);
     for (int it = 0; it < iters; ++it) {
 #pragma unroll
         for (int u = 0; u < kIlp; ++u)
-            asm volatile("red.global.add.v2.f32 [%0], {%1, %2};" ::"l"(buf + path_index(s, lane, nx, nz)), "f"(1.0f), "f"(1.0f) : "memory");
+            asm volatile("red.global.add.v2.f32 [%0], {%1, %2};" ::"l"(buf + path_index<TILED>(s, lane, nx, nz)), "f"(1.0f), "f"(1.0f) : "memory");
     }
 }
 
@@ -168,7 +174,7 @@ struct Timer {
 };
 }  // namespace
 
-extern "C" int pct_measure_peaks(void* stream, int64_t footprint_bytes, double out[8]) {
+extern "C" int pct_measure_peaks(void* stream, int64_t footprint_bytes, double out[12]) {
     if (!out || footprint_bytes < (1 << 20) || footprint_bytes > (1LL << 34)) return PCT_EINVAL;
     cudaStream_t st = (cudaStream_t)stream;
     int dev = 0, sms = 0;
@@ -197,11 +203,15 @@ extern "C" int pct_measure_peaks(void* stream, int64_t footprint_bytes, double o
     int nx = 256;
     while ((uint64_t)nx * nx * 4 > n_words && nx > 16) nx >>= 1;
     const int nz_g = (int)(n_words / ((uint32_t)nx * nx));
-    k_gather_paths<<<grid, 256, 0, st>>>(buf, nx, nz_g, it_g, sink);
+    k_gather_paths<false><<<grid, 256, 0, st>>>(buf, nx, nz_g, it_g, sink);
     T.start();
-    k_gather_paths<<<grid, 256, 0, st>>>(buf, nx, nz_g, it_g, sink);
+    k_gather_paths<false><<<grid, 256, 0, st>>>(buf, nx, nz_g, it_g, sink);
     ms = T.stop_ms();
     out[1] = threads * it_g * kIlp / (ms * 1e-3);
+    T.start();
+    k_gather_paths<true><<<grid, 256, 0, st>>>(buf, nx, nz_g, it_g, sink);
+    ms = T.stop_ms();
+    out[8] = threads * it_g * kIlp / (ms * 1e-3);
     // random 8 B vector reduction
     const int it_r = 128;
     k_red_random<<<grid, 256, 0, st>>>((float2*)buf, n_pairs, it_r);
@@ -211,11 +221,15 @@ extern "C" int pct_measure_peaks(void* stream, int64_t footprint_bytes, double o
     out[2] = threads * it_r * kIlp / (ms * 1e-3);  // reductions/s
     // path-shaped 8 B vector reduction
     const int nz_r = (int)(n_pairs / ((uint32_t)nx * nx));
-    k_red_paths<<<grid, 256, 0, st>>>((float2*)buf, nx, nz_r > 0 ? nz_r : 1, it_r);
+    k_red_paths<false><<<grid, 256, 0, st>>>((float2*)buf, nx, nz_r > 0 ? nz_r : 1, it_r);
     T.start();
-    k_red_paths<<<grid, 256, 0, st>>>((float2*)buf, nx, nz_r > 0 ? nz_r : 1, it_r);
+    k_red_paths<false><<<grid, 256, 0, st>>>((float2*)buf, nx, nz_r > 0 ? nz_r : 1, it_r);
     ms = T.stop_ms();
     out[6] = threads * it_r * kIlp / (ms * 1e-3);
+    T.start();
+    k_red_paths<true><<<grid, 256, 0, st>>>((float2*)buf, nx, nz_r > 0 ? nz_r : 1, it_r);
+    ms = T.stop_ms();
+    out[9] = threads * it_r * kIlp / (ms * 1e-3);
     // streaming 128-bit reads of the footprint
     k_stream_read<<<grid, 256, 0, st>>>((const float4*)buf, bytes / 16, sink);
     T.start();
@@ -235,6 +249,7 @@ extern "C" int pct_measure_peaks(void* stream, int64_t footprint_bytes, double o
     ms = T.stop_ms();
     out[5] = threads * it_f * 64.0 / (ms * 1e-3);  // packed instructions/s (two FMAs each)
     out[7] = (double)bytes;
+    out[10] = out[11] = 0.0;
     cudaError_t e = cudaStreamSynchronize(st);
     if (e == cudaSuccess) e = cudaGetLastError();
     cudaFree(buf);

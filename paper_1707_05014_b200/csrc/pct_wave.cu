@@ -26,13 +26,46 @@
 // Forward progress: a warp holding ticket w waits only for work of tickets < w (held by resident warps, which never
 // wait for a later ticket) and for update sub-tasks, which every waiting warp executes itself.  Every wait is
 // bounded: it gives up after a few seconds, sets ctrl->error and the call reports PCT_EINTERNAL.
+#include <stdio.h>
+#include <string.h>
+
 #include "pct_walk.cuh"
 
 namespace pct {
 
-#ifndef PCT_WAVE_ACQUIRE_PREFETCH
-#define PCT_WAVE_ACQUIRE_PREFETCH 1  // the flag load issued before the walk is ld.acquire (0: relaxed)
+// Build with -DPCT_WAVE_PROF to accumulate, per phase of k_wave, the cycles its warps spent there (a tuning aid:
+// wave_prof_dump prints and clears the totals); the default build carries none of it.
+#ifdef PCT_WAVE_PROF
+__device__ unsigned long long g_wave_prof[16];
+#define PROF_DECL long long prof_t = clock64(); unsigned long long prof_acc[8] = {0, 0, 0, 0, 0, 0, 0, 0}
+#define PROF(i) do { const long long now__ = clock64(); prof_acc[i] += (unsigned long long)(now__ - prof_t); prof_t = now__; } while (0)
+#define PROF_FLUSH do { if (lane == 0) for (int i__ = 0; i__ < 8; ++i__) atomicAdd(&g_wave_prof[i__], prof_acc[i__]); } while (0)
+#define UPROF(i) do { if (stage != nullptr) { const long long now__ = clock64(); if (lane == 0) atomicAdd(&g_wave_prof[8 + (i)], (unsigned long long)(now__ - uprof_t)); uprof_t = now__; } } while (0)
+#define UPROF_DECL long long uprof_t = clock64()
+#define UPROF_COUNT(i) do { if (stage != nullptr && lane == 0) atomicAdd(&g_wave_prof[8 + (i)], 1ULL); } while (0)
+#else
+#define PROF_DECL
+#define PROF(i)
+#define PROF_FLUSH
+#define UPROF(i)
+#define UPROF_DECL
+#define UPROF_COUNT(i)
 #endif
+
+// Warp roles.  The first kWalkers warps of a CTA walk histories; the last kUpdaters warps only run posted update
+// sub-tasks, staged through shared memory with cp.async so that a whole sub-task is ONE memory round trip: an update
+// must be finished long before the next block reaches its slab, and a walker's registers are taken by the walk.
+#ifndef PCT_WAVE_UPDATERS
+#define PCT_WAVE_UPDATERS 2
+#endif
+constexpr int kUpdaters = PCT_WAVE_UPDATERS;
+constexpr int kWalkers = kWarpsPerCta - kUpdaters;
+constexpr int kStageGroups = 256;                // groups of four voxels staged at once by an updater warp
+constexpr int kStageBytes = kStageGroups * 48;   // 32 B of accumulator + 16 B of image per group
+static_assert(kUpdaters >= 1 && kWalkers >= 1, "a CTA needs both roles");
+
+__host__ __device__ inline int wave_stage_off(int nmin) { return (smem_layout(nmin).total + 15) & ~15; }
+static size_t wave_smem_bytes(int nmin) { return (size_t)wave_stage_off(nmin) + (size_t)kUpdaters * kStageBytes; }
 
 __device__ __forceinline__ unsigned ld_acquire_u32(const unsigned* p) {
     unsigned v;
@@ -151,8 +184,8 @@ __device__ __forceinline__ float updated_w(float xv, float d, float c, float lam
 __device__ __forceinline__ void update_subtask(const WaveArgs& a, int s, int sub, int lane) {
     const long long v0 = (long long)s * a.slab_voxels;
     const long long v1 = v0 + a.slab_voxels < a.n_voxels ? v0 + a.slab_voxels : a.n_voxels;
-    if ((a.slab_voxels & 3) == 0) {
-        const long long n4 = (v1 - v0) >> 2;  // (v1 - v0 is a multiple of four: whole slices of nx*ny voxels, nx*ny*slab_slices % 4 == 0)
+    if ((a.g.slice_p & 3) == 0) {  // (always: stored slices have even sides) 128 bits at a time
+        const long long n4 = (v1 - v0) >> 2;
         const long long per = (n4 + a.n_sub - 1) / a.n_sub;
         const long long g0 = (v0 >> 2) + (long long)sub * per;
         const long long g1 = g0 + per < (v0 >> 2) + n4 ? g0 + per : (v0 >> 2) + n4;
@@ -204,89 +237,197 @@ __device__ __forceinline__ void update_subtask(const WaveArgs& a, int s, int sub
     }
 }
 
-// Claim and run one posted update sub-task, if there is one.  Warp-collective.  Returns false iff none was found.
-__device__ __forceinline__ bool try_update(const WaveArgs& a, int lane, unsigned warp_id) {
+// The same sub-task by an updater warp: accumulator and image of up to kStageGroups groups go to shared memory with
+// cp.async (L2 only, no registers: the whole chunk is in flight at once), are combined there and written back.
+__device__ __forceinline__ void update_subtask_staged(const WaveArgs& a, int s, int sub, int lane, float4* stage) {
+    const long long v0 = (long long)s * a.slab_voxels;
+    const long long v1 = v0 + a.slab_voxels < a.n_voxels ? v0 + a.slab_voxels : a.n_voxels;
+    const long long n4 = (v1 - v0) >> 2;
+    const long long per = (n4 + a.n_sub - 1) / a.n_sub;
+    const long long g0 = (v0 >> 2) + (long long)sub * per;
+    const long long g1 = g0 + per < (v0 >> 2) + n4 ? g0 + per : (v0 >> 2) + n4;
+    float4* x4 = reinterpret_cast<float4*>(a.x);
+    float4* a4 = reinterpret_cast<float4*>(a.acc);
+    float4* s_acc = stage;
+    float4* s_x = stage + 2 * kStageGroups;
+    const unsigned sa_acc = (unsigned)__cvta_generic_to_shared(s_acc), sa_x = (unsigned)__cvta_generic_to_shared(s_x);
+    for (long long c0 = g0; c0 < g1; c0 += kStageGroups) {
+        const int ng = g1 - c0 < kStageGroups ? (int)(g1 - c0) : kStageGroups;
+        const float4* ga = a4 + 2 * c0;
+        const float4* gx = x4 + c0;
+        for (int i = lane; i < 2 * ng; i += 32)
+            asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(sa_acc + 16u * (unsigned)i), "l"(ga + i) : "memory");
+        for (int i = lane; i < ng; i += 32)
+            asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(sa_x + 16u * (unsigned)i), "l"(gx + i) : "memory");
+        asm volatile("cp.async.commit_group;\n\tcp.async.wait_group 0;" ::: "memory");
+        __syncwarp();
+        for (int i = lane; i < ng; i += 32) {
+            const float4 a01 = s_acc[2 * i], a23 = s_acc[2 * i + 1];
+            const bool hit01 = a01.y > 0.0f || a01.w > 0.0f, hit23 = a23.y > 0.0f || a23.w > 0.0f;
+            if (hit01 || hit23) {
+                float4 v = s_x[i];
+                v.x = updated_w(v.x, a01.x, a01.y, a.lambda);
+                v.y = updated_w(v.y, a01.z, a01.w, a.lambda);
+                v.z = updated_w(v.z, a23.x, a23.y, a.lambda);
+                v.w = updated_w(v.w, a23.z, a23.w, a.lambda);
+                __stcg(x4 + c0 + i, v);
+                const float4 z = make_float4(0.f, 0.f, 0.f, 0.f);
+                if (hit01) __stcg(a4 + 2 * (c0 + i), z);
+                if (hit23) __stcg(a4 + 2 * (c0 + i) + 1, z);
+            }
+        }
+        __syncwarp();  // the staging buffer is overwritten by the next chunk
+    }
+}
+
+__device__ __forceinline__ unsigned long long ld_relaxed_u64(const unsigned long long* p) {
+    unsigned long long v;
+    asm volatile("ld.relaxed.gpu.global.u64 %0, [%1];" : "=l"(v) : "l"(p) : "memory");
+    return v;
+}
+__device__ __forceinline__ void fence_acq_rel() { asm volatile("fence.acq_rel.gpu;" ::: "memory"); }
+
+__device__ __forceinline__ bool task_open(unsigned long long t) { return (unsigned)(t >> 32) < (unsigned)t; }  // claimed < posted
+
+// Run sub-task `sub` of the update of slab s that was posted last, then count it; the last one of the update
+// publishes upd_seq.  Warp-collective.
+__device__ __noinline__ void run_update(const WaveArgs& a, int s, unsigned sub, int lane, float4* stage) {
     WaveCtrl* c = a.ctrl;
-    unsigned p = 0, cl = 0;
-    if (lane < a.n_slabs) {
-        p = ld_acquire_u32(&c->posted[lane]);
-        cl = ld_relaxed_u32(&c->claimed[lane]);
-    }
-    const unsigned avail = __ballot_sync(0xffffffffu, cl < p * (unsigned)a.n_sub);
-    if (avail == 0u) return false;
-    // the warps spread over the slabs that have work: first available slab at or after a warp-dependent start
-    const unsigned rot = warp_id & 31u;
-    const unsigned hi = avail >> rot;
-    const int s = hi ? (int)rot + __ffs(hi) - 1 : __ffs(avail) - 1;
-    const unsigned mine = __shfl_sync(0xffffffffu, cl, s);
-    int got = 0;
-    if (lane == 0) {
-        got = atomicCAS(&c->claimed[s], mine, mine + 1u) == mine;
-        if (got) atomicSub(&c->pending, 1);
-    }
-    got = __shfl_sync(0xffffffffu, got, 0);
-    if (!got) return true;  // another warp took it; there may be more
-    const unsigned seq = ld_relaxed_u32(&c->post_seq[s]);  // (written before `posted` moved: ordered by the acquire above)
-    update_subtask(a, s, (int)(mine % (unsigned)a.n_sub), lane);
-    __threadfence();  // every lane's stores, before the counter moves
+    // (no fence on this side of the claim: the CAS that won it returned before anything below is issued, and what
+    // follows reads the L2, where post_seq and every reduction of the block were visible before the post)
+    UPROF_DECL;
+    const unsigned seq = ld_relaxed_u32(&c->post_seq[s]);
+    if (stage != nullptr && (a.g.slice_p & 3) == 0)
+        update_subtask_staged(a, s, (int)sub, lane, stage);
+    else
+        update_subtask(a, s, (int)sub, lane);
+    UPROF(1);
+    fence_acq_rel();  // every lane's stores, before the counter moves
     __syncwarp();
+    UPROF(2);
+    UPROF_COUNT(5);
     if (lane == 0) {
         const unsigned f = atomicAdd(&c->finished[s], 1u);
         if ((f + 1u) % (unsigned)a.n_sub == 0u) {  // the last sub-task of this update
-            __threadfence();
+            fence_acq_rel();
             st_release_u32(&c->upd_seq[s], seq + 1u);
         }
     }
+}
+
+// Claim one sub-task of slab s given the task word `t` just read (claimed < posted).  One attempt: a warp that loses
+// the race goes back to its histories (somebody else is at it).  Warp-collective; returns true iff a sub-task was run.
+__device__ __forceinline__ bool claim_and_run(const WaveArgs& a, int s, unsigned long long t, int lane, float4* stage) {
+    int got = 0;
+    if (lane == 0) {
+        // the poster may add to the low half between the load and the CAS: retry once with what the CAS returned
+        unsigned long long seen = atomicCAS(&a.ctrl->tasks[s], t, t + (1ULL << 32));
+        got = seen == t;
+        if (!got && (seen >> 32) == (t >> 32) && task_open(seen)) {
+            t = seen;
+            got = atomicCAS(&a.ctrl->tasks[s], t, t + (1ULL << 32)) == t;
+        }
+    }
+    got = __shfl_sync(0xffffffffu, got, 0);
+    if (!got) return false;
+    run_update(a, s, (unsigned)(t >> 32) % (unsigned)a.n_sub, lane, stage);
+    return true;
+}
+
+// Look at EVERY slab for an open update sub-task and run one (used where the warp has nothing better to do: while it
+// waits for a slab, and after the last work item).  Warp-collective.  Returns false iff nothing was open.
+__device__ __noinline__ bool steal_update(const WaveArgs& a, int lane, unsigned warp_id, float4* stage) {
+    unsigned long long t = 0;
+    if (lane < a.n_slabs) t = ld_relaxed_u64(&a.ctrl->tasks[lane]);
+    const unsigned avail = __ballot_sync(0xffffffffu, task_open(t));
+    if (avail == 0u) return false;
+    const unsigned rot = warp_id & 31u;  // the warps spread over the slabs that have work
+    const unsigned hi = avail >> rot;
+    const int s = hi ? (int)rot + __ffs(hi) - 1 : __ffs(avail) - 1;
+    t = __shfl_sync(0xffffffffu, t, s);
+    claim_and_run(a, s, t, lane, stage);
     return true;
 }
 
 // The update of slab s after block q is due: post its sub-tasks.
 __device__ __forceinline__ void post_update(const WaveArgs& a, int s, unsigned q) {
     WaveCtrl* c = a.ctrl;
-    __threadfence();  // (acquire side of the done[] counter: the other warps' reductions are ordered before what follows)
+    fence_acq_rel();  // (acquire side of the done[] counter: the other warps' reductions are ordered before what follows)
     asm volatile("st.relaxed.gpu.global.u32 [%0], %1;" ::"l"(&c->post_seq[s]), "r"(q) : "memory");
-    __threadfence();
-    atomicAdd(&c->posted[s], 1u);
-    atomicAdd(&c->pending, a.n_sub);
+    fence_acq_rel();
+    atomicAdd(&c->tasks[s], (unsigned long long)a.n_sub);
 }
 
-constexpr unsigned kSpinLimit = 1u << 23;  // x >= 100 ns: a wait gives up after about a second of doing nothing
+constexpr unsigned kSpinLimit = 1u << 20;  // x 2-4 us: a wait gives up after a few seconds of doing nothing
 
-// Wait until slabs [sa, sb] hold the image after blocks [0, q) of the sweep.  Lane l looks after slab sa + l; `flag` is
-// the value of upd_seq it loaded before the walk.  A block without a history for a slab never posts an update for
-// it: whoever waits moves upd_seq over such blocks (need == 0) itself.  While waiting the warp runs update sub-tasks.
-__device__ __forceinline__ bool wait_slabs(const WaveArgs& a, int lane, unsigned warp_id, int sa, int sb, unsigned q, unsigned flag) {
+// Do slabs [sa, sb] hold the image after blocks [0, q) of the sweep?  Lane l looks after slab sa + l (`ok` carries its
+// answer from call to call).  A block without a history for a slab never posts an update for it: whoever asks moves
+// upd_seq over such blocks (need == 0) itself.  Warp-collective.
+__device__ __forceinline__ bool slabs_reached(const WaveArgs& a, int lane, int sa, int sb, unsigned q, bool& ok) {
     WaveCtrl* c = a.ctrl;
-    const bool mine = lane <= sb - sa;
-    bool ok = !mine || flag >= q;
-    if (__all_sync(0xffffffffu, ok)) return true;
-    unsigned spins = 0;
-    for (;;) {
-        if (!ok) {
-            const int s = sa + lane;
-            unsigned u = ld_acquire_u32(&c->upd_seq[s]);
-            if (u < q && __ldg(a.need + (long long)u * a.n_slabs + s) == 0) {
-                atomicCAS(&c->upd_seq[s], u, u + 1u);  // block u has nothing for this slab
-                u = ld_acquire_u32(&c->upd_seq[s]);
-            }
-            ok = u >= q;
+    if (!ok && lane <= sb - sa) {
+        const int s = sa + lane;
+        unsigned u = ld_acquire_u32(&c->upd_seq[s]);
+        while (u < q && __ldg(a.need + (long long)u * a.n_slabs + s) == 0) {
+            atomicCAS(&c->upd_seq[s], u, u + 1u);  // block u has nothing for this slab
+            u = ld_acquire_u32(&c->upd_seq[s]);
         }
-        if (__all_sync(0xffffffffu, ok)) return true;
-        if (!try_update(a, lane, warp_id)) {
-            __nanosleep(100);
-            unsigned err = 0;
-            if (lane == 0) err = ld_relaxed_u32(&c->error) & 2u;
-            err = __shfl_sync(0xffffffffu, err, 0);
-            if (++spins > kSpinLimit || err) {
-                if (lane == 0) atomicOr(&c->error, 2u);
-                return false;
-            }
+        ok = u >= q;
+    }
+    return __all_sync(0xffffffffu, ok || lane > sb - sa);
+}
+
+__device__ __forceinline__ bool wave_failed(WaveCtrl* c, int lane) {
+    unsigned err = 0;
+    if (lane == 0) err = ld_relaxed_u32(&c->error) & 2u;
+    return __shfl_sync(0xffffffffu, err, 0) != 0u;
+}
+
+// A walker waits for the slabs of the history it has just walked.  The updater warps do the updates; a walker that
+// has waited for a while lends a hand (register path), which also keeps the launch alive whatever is resident.
+__device__ __noinline__ bool wait_slabs_slow(const WaveArgs& a, int lane, unsigned warp_id, int sa, int sb, unsigned q) {
+    bool ok = false;
+    for (unsigned spins = 0;; ++spins) {
+        if (slabs_reached(a, lane, sa, sb, q, ok)) return true;
+        if (spins >= 8u && steal_update(a, lane, warp_id, nullptr)) continue;
+        // back off: thousands of warps may wait on the same few words, and an update takes microseconds
+        __nanosleep(spins < 4u ? (250u << spins) : 4000u);
+        if (spins > kSpinLimit || ((spins & 63u) == 63u && wave_failed(a.ctrl, lane))) {
+            if (lane == 0) atomicOr(&a.ctrl->error, 2u);
+            return false;
+        }
+    }
+}
+
+// `flag`: the value of upd_seq[sa + lane] loaded before the walk (the common case: long up to date).
+__device__ __forceinline__ bool wait_slabs(const WaveArgs& a, int lane, unsigned warp_id, int sa, int sb, unsigned q, unsigned flag) {
+    const bool ok = lane > sb - sa || flag >= q;
+    if (__all_sync(0xffffffffu, ok)) return true;
+    return wait_slabs_slow(a, lane, warp_id, sa, sb, q);
+}
+
+// An updater warp: run posted update sub-tasks until every slab holds the image after block q1 - 1.
+__device__ __noinline__ void updater_loop(const WaveArgs& a, int lane, unsigned warp_id, float4* stage) {
+    bool ok = false;
+    UPROF_DECL;
+    for (unsigned idle = 0;;) {
+        if (steal_update(a, lane, warp_id, stage)) {
+            idle = 0;
+            UPROF(3);
+            continue;
+        }
+        UPROF(4);
+        if ((idle & 3u) == 0u && slabs_reached(a, lane, 0, a.n_slabs - 1, (unsigned)a.q1, ok)) return;
+        __nanosleep(idle < 3u ? (250u << idle) : 2000u);
+        if (++idle > kSpinLimit || ((idle & 63u) == 63u && wave_failed(a.ctrl, lane))) {
+            if (lane == 0) atomicOr(&a.ctrl->error, 2u);
+            return;
         }
     }
 }
 
 template <bool SPLINE>
-__global__ void __launch_bounds__(kThreads, kCtasPerSm) k_wave(const WaveArgs a) {
+__global__ void __launch_bounds__(kThreads, kCtasPerSm) k_wave(const __grid_constant__ WaveArgs a) {
     extern __shared__ __align__(16) unsigned char smem_raw[];
     const Geom g = a.g;
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
@@ -298,23 +439,20 @@ __global__ void __launch_bounds__(kThreads, kCtasPerSm) k_wave(const WaveArgs a)
     stage_table(s_tab, a.tab, g.nmin);
     WaveCtrl* ctrl = a.ctrl;
     const bool planned = a.plan != nullptr;
+    if (warp >= kWalkers) {  // updater warps (no CTA-wide barrier follows)
+        if (planned)
+            updater_loop(a, lane, warp_id, reinterpret_cast<float4*>(smem_raw + wave_stage_off(g.nmin)) + (warp - kWalkers) * (kStageBytes / 16));
+        return;
+    }
     const long long B = planned ? a.block_size : a.count;
     const long long ipb = (B + a.item - 1) / a.item;  // items per block
     const unsigned long long n_items = planned ? (unsigned long long)(a.q1 - a.q0) * ipb : (unsigned long long)ipb;
     unsigned long long rows = 0, nnz_total = 0, segs = 0;
     const EmitPtrs no_emit{nullptr, nullptr, nullptr, nullptr};
     bool give_up = false;
+    PROF_DECL;
 
     while (!give_up) {
-        if (planned) {  // posted updates first: other warps wait for them
-            int pend = 0;
-            if (lane == 0) pend = (int)ld_relaxed_u32(reinterpret_cast<const unsigned*>(&ctrl->pending));
-            pend = __shfl_sync(0xffffffffu, pend, 0);
-            while (pend > 0 && try_update(a, lane, warp_id)) {
-                if (lane == 0) pend = (int)ld_relaxed_u32(reinterpret_cast<const unsigned*>(&ctrl->pending));
-                pend = __shfl_sync(0xffffffffu, pend, 0);
-            }
-        }
         unsigned long long w = 0;
         if (lane == 0) w = atomicAdd(&ctrl->ticket, 1ULL);
         w = __shfl_sync(0xffffffffu, w, 0);
@@ -337,22 +475,22 @@ __global__ void __launch_bounds__(kThreads, kCtasPerSm) k_wave(const WaveArgs a)
             setup_history(g, hh, s_state[lane]);
         }
         __syncwarp();
+        PROF(0);
         for (int p = 0; p < cnt && !give_up; ++p) {
             const PathState& S = s_state[p];
             const int K = S.K;
             if (K < 0) continue;  // skipped history: empty row (R7)
             const int sa = __shfl_sync(0xffffffffu, my_sa, p), sb = __shfl_sync(0xffffffffu, my_sb, p);
+            // Issued before the walk, used after it (no latency in the warp's way): the flags of the history's slabs.
+            // Relaxed loads: the gather below is issued only
+            // after a flag value >= q has arrived, and it reads the L2, where the updater's stores were visible
+            // before its release of the flag.
             unsigned flag = 0xffffffffu;
-            if (planned && lane <= sb - sa) {
-#if PCT_WAVE_ACQUIRE_PREFETCH
-                flag = ld_acquire_u32(&ctrl->upd_seq[sa + lane]);
-#else
-                flag = ld_relaxed_u32(&ctrl->upd_seq[sa + lane]);
-#endif
-            }
+            if (planned && lane <= sb - sa) flag = ld_relaxed_u32(&ctrl->upd_seq[sa + lane]);
             float nrm;
             int nnz;
             walk_history<false, SPLINE>(g, S, s_tab, lane, row, nrm, nnz, no_emit);
+            PROF(1);
             const int C = (K + 32) >> 5;
             unsigned lo = 0u, span = 0xffffffffu;
             if (planned) {
@@ -363,10 +501,12 @@ __global__ void __launch_bounds__(kThreads, kCtasPerSm) k_wave(const WaveArgs a)
                 lo = (unsigned)((long long)sa * a.slab_voxels);
                 span = (unsigned)((long long)(sb - sa + 1) * a.slab_voxels);
             }
+            PROF(2);
             bool bad = false;
             float dot = gather_row_cg(row, lane, C, a.x, lo, span, bad);
             dot = warp_sum(dot);
             nrm = warp_sum(nrm);
+            PROF(3);
             if (__any_sync(0xffffffffu, bad)) {  // the plan's range does not hold the row: never scatter outside it
                 if (lane == 0) atomicOr(&ctrl->error, 1u);
             } else if (nrm > 0.0f) {  // non-empty row (R13)
@@ -377,16 +517,11 @@ __global__ void __launch_bounds__(kThreads, kCtasPerSm) k_wave(const WaveArgs a)
             }
             __syncwarp();  // the row buffer is reused by the next history
             segs += (lane == 0) ? (K + 1) : 0;
-            if (planned && p + 1 < cnt) {  // an update posted meanwhile? (one load per history)
-                int pend = 0;
-                if (lane == 0) pend = (int)ld_relaxed_u32(reinterpret_cast<const unsigned*>(&ctrl->pending));
-                pend = __shfl_sync(0xffffffffu, pend, 0);
-                if (pend > 0) try_update(a, lane, warp_id);
-            }
+            PROF(4);
         }
         if (planned) {
             // the item has scattered: every lane's reductions are ordered before the counters move
-            __threadfence();
+            fence_acq_rel();
             __syncwarp();
             int mine = 0;  // histories of the item whose range holds slab `lane`
             for (int p = 0; p < cnt; ++p) {
@@ -400,11 +535,14 @@ __global__ void __launch_bounds__(kThreads, kCtasPerSm) k_wave(const WaveArgs a)
             }
         }
         __syncwarp();  // the state records are reused by the next item
+        PROF(6);
     }
     if (planned && !give_up) {
         // no work left to draw: run update sub-tasks until every slab holds the image after block q1 - 1
         wait_slabs(a, lane, warp_id, 0, a.n_slabs - 1, (unsigned)a.q1, 0u);
     }
+    PROF(7);
+    PROF_FLUSH;
     nnz_total = (unsigned long long)__reduce_add_sync(0xffffffffu, (unsigned)nnz_total);
     if (lane == 0) {
         atomicAdd(&ctrl->cur[0], rows);
@@ -412,6 +550,28 @@ __global__ void __launch_bounds__(kThreads, kCtasPerSm) k_wave(const WaveArgs a)
         atomicAdd(&ctrl->cur[2], segs);
     }
 }
+
+void wave_prof_dump(const char* tag) {
+#ifdef PCT_WAVE_PROF
+    unsigned long long h[16] = {0};
+    cudaMemcpyFromSymbol(h, g_wave_prof, sizeof(h));
+    double tot = 0;
+    for (int i = 0; i < 8; ++i) tot += (double)h[i];
+    static const char* names[8] = {"ticket+setup", "walk", "wait", "gather", "scatter", "updates", "signal", "drain"};
+    fprintf(stderr, "[wave prof %s]", tag);
+    for (int i = 0; i < 8; ++i) fprintf(stderr, " %s %.1f%%", names[i], tot > 0 ? 100.0 * (double)h[i] / tot : 0.0);
+    fprintf(stderr, " (total %.3g warp-cycles)\n", tot);
+    fprintf(stderr, "[wave prof updaters] sub-tasks %llu, cycles per sub-task: body %.0f, fence %.0f; loop busy %.3g, idle %.3g warp-cycles\n", h[13],
+            h[13] ? (double)h[9] / h[13] : 0.0, h[13] ? (double)h[10] / h[13] : 0.0, (double)h[11], (double)h[12]);
+    memset(h, 0, sizeof(h));
+    cudaMemcpyToSymbol(g_wave_prof, h, sizeof(h));
+#else
+    (void)tag;
+#endif
+}
+
+int wave_walkers_per_cta() { return kWalkers; }
+size_t wave_smem_need(int nmin) { return wave_smem_bytes(nmin); }
 
 WaveShape wave_shape(const Geom& g) {
     WaveShape s;
@@ -422,16 +582,16 @@ WaveShape wave_shape(const Geom& g) {
     if (s.slab_slices < 1) s.slab_slices = 1;
     if (s.slab_slices > g.nz) s.slab_slices = g.nz;
     s.n_slabs = (g.nz + s.slab_slices - 1) / s.slab_slices;
-    // sub-tasks of about 2048 groups of four voxels (64 per lane)
-    const long long groups = (long long)s.slab_slices * g.nx * g.ny / 4;
-    long long ns = (groups + 2047) / 2048;
+    // sub-tasks of about kStageGroups groups of four voxels: one staged chunk of an updater warp
+    const long long groups = (long long)s.slab_slices * g.slice_p / 4;
+    long long ns = (groups + kStageGroups - 1) / kStageGroups;
     s.n_sub = ns < 1 ? 1 : (ns > 256 ? 256 : (int)ns);
     return s;
 }
 
 cudaError_t wave_configure(int nmin, int* grid_out) {
     if (((nmin + 32) >> 5) > 64) return cudaErrorInvalidValue;
-    const size_t smem = drop_smem_bytes(nmin);
+    const size_t smem = wave_smem_bytes(nmin);
     int dev = 0, sms = 0, per_sm = 0;
     cudaError_t e;
     if ((e = cudaGetDevice(&dev)) != cudaSuccess) return e;
@@ -450,9 +610,9 @@ cudaError_t launch_wave(const WaveArgs& a, int grid, cudaStream_t stream) {
     const long long B = a.plan ? a.block_size : a.count;
     const long long ipb = (B + a.item - 1) / a.item;
     const long long items = a.plan ? (a.q1 - a.q0) * ipb : ipb;
-    const long long need = (items + kWarpsPerCta - 1) / kWarpsPerCta;
+    const long long need = (items + kWalkers - 1) / kWalkers;
     if (need < grid) grid = need < 1 ? 1 : (int)need;
-    const size_t smem = drop_smem_bytes(a.g.nmin);
+    const size_t smem = wave_smem_bytes(a.g.nmin);
     if (a.g.path_model == 1)
         k_wave<true><<<grid, kThreads, smem, stream>>>(a);
     else

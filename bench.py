@@ -38,11 +38,18 @@ OPS_PER_SEGMENT = 106
 HBM_BYTES_PER_HISTORY = 38
 SM_COUNT = 148
 LANES_PER_SM = 128
-# dram__bytes_read.sum + dram__bytes_write.sum of ONE k_drop_block launch, from the committed
-# `ncu --set full` capture profiles/r1d_ncu_full.md (95.0 MB + 57.1 MB; ncu flushes the caches before the
-# replay), keyed by (config, block size); the same launch with warm caches (profiles/r1d_dram_warm.md).
-NCU_DRAM_BYTES_PER_LAUNCH = {(3, 100000): 152.1e6}
-NCU_DRAM_BYTES_PER_LAUNCH_WARM = {(3, 100000): 145.6e6}
+# dram__bytes_read.sum + dram__bytes_write.sum of ONE k_drop_block launch come from the committed ncu captures of
+# THIS build, recorded in profiles/traffic.json (file, commit, bytes per launch with ncu's cache flush and with
+# --cache-control none), keyed by "config:block_size".
+TRAFFIC_JSON = os.path.join(ROOT, "profiles", "traffic.json")
+
+
+def ncu_traffic(config, block_size):
+    try:
+        with open(TRAFFIC_JSON) as f:
+            return json.load(f).get("%d:%d" % (config, block_size))
+    except (OSError, ValueError):
+        return None
 
 
 def parse_args():
@@ -56,6 +63,11 @@ def parse_args():
     ap.add_argument("--e2e-steps", type=int, default=2)
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu", action="store_true")
+    ap.add_argument("--no-peaks", action="store_true", help="skip the L2 / fp32 micro-benchmarks behind roofline.l2")
+    ap.add_argument("--peaks", action="store_true", help="only run the micro-benchmarks (pct_measure_peaks) and print them")
+    ap.add_argument("--time-ordered", action="store_true",
+                    help="histories in acquisition order (a block is nearly single-angle: the scanner rotates continuously, "
+                         "PAPER.md:78) instead of interleaved angles; a sensitivity measurement (SURVEY.md 8(d))")
     ap.add_argument("--cpu-seconds", type=float, default=15.0, help="target CPU time of the oracle sample")
     ap.add_argument("--path-model", default="mlp", choices=["mlp", "spline"],
                     help="spline: the cubic-spline path model (SURVEY.md 8(f) NEXT-3), a side measurement; the metric's is mlp")
@@ -222,11 +234,26 @@ def run_ours(args):
     B, lam, M = cfg.block_size, cfg.lam, cfg.n_voxels
     n_blocks = (n + B - 1) // B
 
+    if args.time_ordered:
+        n -= n % cfg.n_angles
+        n_blocks = (n + B - 1) // B
     # replicas only: rank r draws histories [r*n, (r+1)*n) of the same seeded stream
     D = cuda_gen.generate_cuda(cfg, n, first=replicas.shard_first(rank, n))
+    if args.time_ordered:
+        # the generator interleaves the angles (history i belongs to projection i mod n_angles); acquisition order is
+        # projection after projection: a transpose of the (n / n_angles, n_angles) view of every field
+        for k in list(D):
+            if k not in ("proj_cos", "proj_sin"):
+                D[k] = D[k].view(n // cfg.n_angles, cfg.n_angles).t().contiguous().view(-1)
     P = synth.to_pct_names(D)
     stream = torch.cuda.Stream()
     out = {}
+    if rank == 0 and not args.no_peaks:
+        # the L2 / fp32 denominators of the roofline, measured on THIS GPU before the timed region (a second or two):
+        # on an L2-resident footprint (32 MB) and on the footprint of image + accumulator of the workload
+        torch.cuda.synchronize()
+        out["peaks_l2"] = pct.pct_measure_peaks(32 << 20)
+        out["peaks_ws"] = pct.pct_measure_peaks(max(1 << 20, 12 * M))
     with torch.cuda.stream(stream):  # torch.cuda.Event records on this stream, the one the kernels run on
         ctx = pct.pct_create(cfg.nx, cfg.ny, cfg.nz, cfg.h, cfg.u_in, cfg.u_out, stream.cuda_stream)
         try:
@@ -335,25 +362,58 @@ def run_ours(args):
     alu_ach = ops / (k_ms * 1e-3) / 1e12
     hbm_ach = HBM_BYTES_PER_HISTORY * hist_per_launch / (k_ms * 1e-3) / 1e9
     l2_bytes = (4.0 * seg_per_hist + 8.0 * nnz_per_hist) * hist_per_launch
-    roofline = {
-        "kernel": "pct::k_drop_block (fused hull+MLP+walk+projection+scatter)", "bound": "alu",
-        "achieved": alu_ach, "peak": alu_peak, "unit": "Tinst/s", "frac": alu_ach / alu_peak,
-        "peak_source": "148 SM x 128 fp32 lanes x %.0f MHz (MEASURED_PEAKS.json sm_max_mhz, %s)" % (peaks["sm_max_mhz"], peaks["source"]),
-        "algorithmic": "%d fp32/int ops per path segment (DESIGN.md Roofline) x %.1f segments/history x %d histories/launch" % (
-            OPS_PER_SEGMENT, seg_per_hist, hist_per_launch),
+    traffic = ncu_traffic(args.config, B) or {}
+    t_kernel = k_ms * 1e-3
+    alu = {"achieved": alu_ach, "peak": alu_peak, "unit": "Tinst/s", "frac": alu_ach / alu_peak,
+           "peak_source": "148 SM x 128 fp32 lanes x %.0f MHz (MEASURED_PEAKS.json sm_max_mhz, %s)" % (peaks["sm_max_mhz"], peaks["source"]),
+           "algorithmic": "%d fp32/int ops per path segment (DESIGN.md Roofline) x %.1f segments/history x %d histories/launch" % (
+               OPS_PER_SEGMENT, seg_per_hist, hist_per_launch),
+           "time_at_peak_us": ops / (alu_peak * 1e12) * 1e6}
+    hbm = {"achieved": hbm_ach, "peak": peaks["hbm_gbs"], "unit": "GB/s", "frac": hbm_ach / peaks["hbm_gbs"],
+           "peak_source": "MEASURED_PEAKS.json hbm_gbs (%s)" % peaks["source"], "algorithmic": "38 B/history",
+           "time_at_peak_us": HBM_BYTES_PER_HISTORY * hist_per_launch / (peaks["hbm_gbs"] * 1e9) * 1e6}
+    common = {
+        "kernel": "pct::k_drop_block (fused hull+MLP+walk+projection+scatter)",
         "kernel_ms": k_ms, "launches_timed": prof["blocks"],
         "kernel_share_of_step": prof["accumulate_ms"] / prof["sweep_ms"],
         "update_kernel_ms": prof["update_ms"] / prof["blocks"],
         "timing": "CUDA events around every launch on the kernels' stream (pct_profile_sweep), one sweep of the timed workload",
-        "traffic": NCU_DRAM_BYTES_PER_LAUNCH.get((args.config, B)),
-        "traffic_source": "profiles/r1d_ncu_full.md (ncu --set full, bytes of DRAM per launch, caches flushed by ncu)",
-        "traffic_warm": NCU_DRAM_BYTES_PER_LAUNCH_WARM.get((args.config, B)),
-        "traffic_warm_source": "profiles/r1d_dram_warm.md (ncu --cache-control none)",
-        "hbm": {"achieved": hbm_ach, "peak": peaks["hbm_gbs"], "unit": "GB/s", "frac": hbm_ach / peaks["hbm_gbs"],
-                "peak_source": peaks["source"], "algorithmic": "38 B/history"},
-        "l2_useful": {"achieved": l2_bytes / (k_ms * 1e-3) / 1e9, "unit": "GB/s",
-                      "algorithmic": "4 B gather/segment + 8 B (Delta,c) reduction/non-zero"},
+        "traffic": traffic.get("cold_bytes"), "traffic_warm": traffic.get("warm_bytes"),
+        "traffic_source": "%s (commit %s): dram__bytes_read.sum + dram__bytes_write.sum of one launch, ncu --set full (caches flushed) / "
+                          "--cache-control none (warm)" % (traffic.get("file"), traffic.get("commit")) if traffic else None,
+        "alu": alu, "hbm": hbm,
     }
+    if "peaks_l2" in out:
+        pk, pw = out["peaks_l2"], out["peaks_ws"]
+        rg, rr = pk["gather_path_tiled_per_s"], pk["red_v2_path_tiled_per_s"]
+        t_peak_hist = seg_per_hist / rg + nnz_per_hist / rr  # seconds per history at the measured L2 rates
+        l2_peak = l2_bytes / hist_per_launch / t_peak_hist / 1e9
+        l2_ach = l2_bytes / t_kernel / 1e9
+        alu_meas = pk["ffma_inst_per_s"] / 1e12
+        alu["peak_measured_ffma"] = alu_meas
+        alu["frac_of_measured_ffma"] = alu_ach / alu_meas
+        times = {"l2": t_peak_hist * hist_per_launch * 1e6, "alu": alu["time_at_peak_us"], "hbm": hbm["time_at_peak_us"]}
+        roofline = dict(common)
+        roofline.update({
+            "bound": "l2", "achieved": l2_ach, "peak": l2_peak, "unit": "GB/s", "frac": l2_ach / l2_peak,
+            "algorithmic": "4 B gather per path segment + 8 B (Delta, c) reduction per non-zero: %.1f segments, %.1f non-zeros per "
+                           "history = %.0f B/history x %d histories/launch" % (seg_per_hist, nnz_per_hist, l2_bytes / hist_per_launch,
+                                                                                hist_per_launch),
+            "peak_source": "measured in this run, before the timed region (pct_measure_peaks, 32 MiB = L2-resident, accesses shaped like "
+                           "the row passes, voxels in the library's 2x2 tiles): %.0f G gathers/s, %.0f G reductions/s; peak = the same "
+                           "bytes at those rates" % (rg / 1e9, rr / 1e9),
+            "binds": max(times, key=times.get), "time_at_peak_us": times,
+            "l2_rates_on_working_set": {"footprint_bytes": pw["footprint_bytes"],
+                                        "gather_path_tiled_per_s": pw["gather_path_tiled_per_s"],
+                                        "red_v2_path_tiled_per_s": pw["red_v2_path_tiled_per_s"],
+                                        "note": "the same micro-benchmarks on image + accumulator of this workload (not L2-resident "
+                                                "when above ~64 MB): context, not the peak"},
+            "peaks_measured": pk,
+        })
+    else:
+        roofline = dict(common)
+        roofline.update({"bound": "alu", "achieved": alu_ach, "peak": alu_peak, "unit": "Tinst/s", "frac": alu_ach / alu_peak,
+                         "peak_source": alu["peak_source"], "algorithmic": alu["algorithmic"]})
     line = {
         "metric": METRIC, "value": out["value"], "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
         "ms_per_step": out["ms_per_step"], "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
@@ -364,6 +424,8 @@ def run_ours(args):
                    "l2": "inputs larger than L2 (histories %.1f GB, image+accumulator %.0f MB vs 126 MB L2)" % (
                        38.0 * n / 1e9, 12.0 * M / 1e6),
                    "multi_gpu": "replicas only", "histories_override": args.histories is not None,
+                   "history_order": "acquisition order, projection after projection (sensitivity run)" if args.time_ordered
+                   else "angles interleaved (every block sees every angle)",
                    "path_model": "most-likely path (the metric's)" if args.path_model == "mlp"
                    else "cubic spline (side measurement, SURVEY.md 8(f) NEXT-3; the roofline's op count is the MLP's)"},
         "clocks": out["clocks"], "gpu_launches": 2 * n_blocks * args.steps,
@@ -417,9 +479,28 @@ def run_carp(args):
                                  "step": "one CARP iteration: every string one DROP sweep over its histories, then the mean"}}))
 
 
+def run_peaks(args):
+    """Only the micro-benchmarks behind roofline.l2 (pct_measure_peaks), on an L2-resident footprint and on the
+    footprint of image + accumulator of the config."""
+    import torch
+
+    import paper_1707_05014_b200 as pct
+    import synth
+
+    cfg = synth.config(args.config)
+    torch.cuda.set_device(0)
+    torch.zeros(1, device="cuda")
+    res = {"config": cfg.workload}
+    for name, fp in (("l2_resident_32MiB", 32 << 20), ("image_plus_accumulator", max(1 << 20, 12 * cfg.n_voxels))):
+        res[name] = pct.pct_measure_peaks(fp)
+    print(json.dumps(res))
+
+
 def main():
     args = parse_args()
-    if args.carp_strings > 0 and args.impl != "reference":
+    if args.peaks:
+        run_peaks(args)
+    elif args.carp_strings > 0 and args.impl != "reference":
         run_carp(args)
     elif args.impl == "reference":
         run_reference(args)

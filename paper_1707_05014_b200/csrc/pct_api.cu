@@ -513,7 +513,7 @@ static DropArgs drop_args(pct_ctx* c, long long block_size, long long first, lon
 
 static int enqueue_pair(pct_ctx* c, const DropArgs& a, float lambda, long long n_blocks, cudaStream_t s) {
     CUDA_TRY(c, launch_drop_block(a, c->drop_grid, s));
-    CUDA_TRY(c, launch_update(c->x, c->acc, c->n_slots, lambda, c->ctrl, n_blocks, s));
+    CUDA_TRY(c, launch_update(c->x, c->acc, c->n_slots, lambda, c->ctrl, n_blocks, c->order != nullptr, s));
     return PCT_OK;
 }
 
@@ -801,7 +801,7 @@ extern "C" int pct_iterate_carp(pct_ctx* c, float lambda, int64_t block_size, in
             const int grid = (c->drop_grid + P - 1) / P;
             for (long long b = 0; b < n_blocks; ++b) {
                 CUDA_TRY(c, launch_drop_block(a, grid, s));
-                CUDA_TRY(c, launch_update(xs, a.acc, M, lambda, a.ctrl, n_blocks, s));
+                CUDA_TRY(c, launch_update(xs, a.acc, M, lambda, a.ctrl, n_blocks, c->order != nullptr, s));
             }
             CUDA_TRY(c, cudaEventRecord(c->carp_done[p], s));
             CUDA_TRY(c, cudaStreamWaitEvent(c->stream, c->carp_done[p], 0));
@@ -969,7 +969,7 @@ extern "C" int pct_profile_sweep(pct_ctx* c, float lambda, int64_t block_size, f
             for (int i = 0; i < nb; ++i) {
                 CUDA_TRY(c, launch_drop_block(a, c->drop_grid, c->stream));
                 CUDA_TRY(c, cudaEventRecord(ev[2 * i + 1], c->stream));
-                CUDA_TRY(c, launch_update(c->x, c->acc, c->n_slots, lambda, c->ctrl, n_blocks, c->stream));
+                CUDA_TRY(c, launch_update(c->x, c->acc, c->n_slots, lambda, c->ctrl, n_blocks, c->order != nullptr, c->stream));
                 CUDA_TRY(c, cudaEventRecord(ev[2 * i + 2], c->stream));
             }
             CUDA_TRY(c, cudaStreamSynchronize(c->stream));

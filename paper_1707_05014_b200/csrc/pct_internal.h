@@ -55,7 +55,7 @@ size_t drop_smem_bytes(int nmin);
 cudaError_t drop_configure(int nmin, int* grid_out);
 cudaError_t launch_drop_block(const DropArgs& a, int grid, cudaStream_t stream);
 cudaError_t launch_update(float* x, float2* acc, long long n_voxels, float lambda, Ctrl* ctrl,
-                          long long n_blocks, cudaStream_t stream);
+                          long long n_blocks, bool top_down, cudaStream_t stream);
 cudaError_t launch_split_acc(float2* acc, float* delta, float* cnt, const Geom& g, cudaStream_t stream);
 cudaError_t launch_image_io(float* x, float* ext, const Geom& g, bool to_storage, cudaStream_t stream);
 cudaError_t launch_rows(const RowsArgs& a, cudaStream_t stream);

@@ -13,6 +13,8 @@
 //                 path is computed once per sweep and never touches global memory.
 //   k_update      x_j += lambda * Delta_j / max(1, c_j); accumulator zeroed; DROP block index advanced.
 //   k_rows        inspection: the same walk, rows written out instead of consumed.
+#include <stdlib.h>
+
 #include "pct_walk.cuh"
 
 namespace pct {
@@ -117,6 +119,13 @@ __global__ void __launch_bounds__(kThreads, kCtasPerSm) k_drop_block(const DropA
     PathState* s_state = reinterpret_cast<PathState*>(smem_raw + lay.state_off) + warp * kBatch;
     float2* row = reinterpret_cast<float2*>(smem_raw + lay.row_off) + warp * lay.row_slots;
     __shared__ Queue q;  // one copy per CTA: the phase of a ticket is looked up by index
+    // Programmatic dependent launch: this grid may start while the update kernel of the previous block is still
+    // running (its CTAs take the SM slots the update's CTAs leave).  The table does not depend on it; everything
+    // else -- the block index in ctrl, the image -- is read after the wait below, i.e. after that grid has completed
+    // and its writes are visible.
+    asm volatile("griddepcontrol.launch_dependents;" ::: "memory");  // the update kernel may take the slots this grid's CTAs leave
+    stage_table(s_tab, a.tab, g.nmin);
+    asm volatile("griddepcontrol.wait;" ::: "memory");
     if (threadIdx.x == 0) {
         long long first = a.first, count = a.count;
         if (first < 0) {
@@ -126,7 +135,7 @@ __global__ void __launch_bounds__(kThreads, kCtasPerSm) k_drop_block(const DropA
         q = make_queue(first, count, (long long)gridDim.x * kWarpsPerCta);
         q.interleave = a.first < 0 && a.order != nullptr;
     }
-    stage_table(s_tab, a.tab, g.nmin);  // (ends with __syncthreads: q is visible)
+    __syncthreads();  // q is visible
     unsigned long long rows = 0, nnz_total = 0, segs = 0;
     const EmitPtrs no_emit{nullptr, nullptr, nullptr, nullptr};
 
@@ -194,17 +203,42 @@ cudaError_t drop_configure(int nmin, int* grid_out) {
     return cudaSuccess;
 }
 
+// Launch with the programmatic-stream-serialization attribute: the grid may be scheduled as soon as the previous
+// kernel in the stream lets its SM slots go; the kernel itself waits (griddepcontrol.wait) before it reads anything
+// the previous kernel writes.  PCT_PDL=0 launches the plain way.
+static bool pdl_enabled() {
+    static int on = -1;
+    if (on < 0) {
+        const char* env = getenv("PCT_PDL");
+        on = (env && env[0] == '0') ? 0 : 1;
+    }
+    return on == 1;
+}
+
+template <typename... KArgs, typename... Args>
+static cudaError_t launch_pdl(void (*kernel)(KArgs...), dim3 grid, dim3 block, size_t smem, cudaStream_t stream, Args... args) {
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = grid;
+    cfg.blockDim = block;
+    cfg.dynamicSmemBytes = smem;
+    cfg.stream = stream;
+    cudaLaunchAttribute attr[1];
+    attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+    attr[0].val.programmaticStreamSerializationAllowed = 1;
+    cfg.attrs = attr;
+    cfg.numAttrs = pdl_enabled() ? 1 : 0;
+    return cudaLaunchKernelEx(&cfg, kernel, args...);
+}
+
 cudaError_t launch_drop_block(const DropArgs& a, int grid, cudaStream_t stream) {
     // never more warps than histories (small blocks: one history per warp)
     const long long cnt = a.first < 0 ? a.block_size : a.count;
     const long long need = (cnt + kWarpsPerCta - 1) / kWarpsPerCta;
     if (need < grid) grid = need < 1 ? 1 : (int)need;
     const size_t smem = drop_smem_bytes(a.g.nmin);
-    if (a.g.path_model == 1)
-        k_drop_block<true><<<grid, kThreads, smem, stream>>>(a);
-    else
-        k_drop_block<false><<<grid, kThreads, smem, stream>>>(a);
-    return cudaGetLastError();
+    cudaError_t e = a.g.path_model == 1 ? launch_pdl(k_drop_block<true>, dim3(grid), dim3(kThreads), smem, stream, a)
+                                        : launch_pdl(k_drop_block<false>, dim3(grid), dim3(kThreads), smem, stream, a);
+    return e != cudaSuccess ? e : cudaGetLastError();
 }
 
 // x_j += lambda * Delta_j / max(1, c_j) (R12); c_j >= 1 wherever anything was accumulated.
@@ -233,9 +267,14 @@ __device__ __forceinline__ void st4_hint(float4* p, float4 v, unsigned long long
 // One group = four consecutive voxels: two 128-bit accumulator loads, one 128-bit image load.  A
 // thread issues the loads of PCT_UPD_UNROLL groups (a CTA-stride apart, so that every load is
 // coalesced) before it touches any of them: the kernel is bound by L2 latency x bytes in flight.
+// top_down: sweep the image from the last slice to the first.  With the histories of a block taken depth slab by
+// depth slab (k_order_blocks) the accumulate kernel ends on the last slabs and the next one starts on the first: the
+// update then finds the end of image and accumulator still in the L2 and leaves their beginning there.
 __global__ void __launch_bounds__(256) k_update(float* __restrict__ x, float2* __restrict__ acc, long long n_voxels,
-                                                float lambda, Ctrl* ctrl, long long n_blocks) {
+                                                float lambda, Ctrl* ctrl, long long n_blocks, bool top_down) {
     constexpr int UN = PCT_UPD_UNROLL;
+    asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
+    asm volatile("griddepcontrol.wait;" ::: "memory");  // (launched while the accumulate kernel of the block drains: see launch_pdl)
     const unsigned long long keep = policy_evict_last();
 #if PCT_ACC_EVICT_FIRST
     const unsigned long long stream_pol = policy_evict_first();
@@ -251,8 +290,9 @@ __global__ void __launch_bounds__(256) k_update(float* __restrict__ x, float2* _
         float4 a01[UN], a23[UN], xv[UN];
 #pragma unroll
         for (int u = 0; u < UN; ++u) {
-            const long long q = q0 + u * stride;
+            long long q = q0 + u * stride;
             if (q < n4) {
+                if (top_down) q = n4 - 1 - q;
                 a01[u] = PCT_LD_ACC(a4 + 2 * q);
                 a23[u] = PCT_LD_ACC(a4 + 2 * q + 1);
                 xv[u] = ld4_hint(x4 + q, keep);
@@ -262,7 +302,8 @@ __global__ void __launch_bounds__(256) k_update(float* __restrict__ x, float2* _
         }
 #pragma unroll
         for (int u = 0; u < UN; ++u) {
-            const long long q = q0 + u * stride;
+            long long q = q0 + u * stride;
+            if (top_down) q = n4 - 1 - q;
             const bool hit01 = a01[u].y > 0.0f || a01[u].w > 0.0f, hit23 = a23[u].y > 0.0f || a23[u].w > 0.0f;
             if (hit01 || hit23) {  // (q < n4 is implied: out-of-range groups were loaded as zeros)
                 float4 v = xv[u];
@@ -302,14 +343,14 @@ __global__ void __launch_bounds__(256) k_update(float* __restrict__ x, float2* _
 }
 
 cudaError_t launch_update(float* x, float2* acc, long long n_voxels, float lambda, Ctrl* ctrl, long long n_blocks,
-                          cudaStream_t stream) {
+                          bool top_down, cudaStream_t stream) {
     const long long n4 = n_voxels >> 2;
     long long blocks = (n4 + 256 * PCT_UPD_UNROLL - 1) / (256 * PCT_UPD_UNROLL);
     if (blocks < 1) blocks = 1;
     const long long cap = (long long)sm_count() * PCT_UPD_CTAS;
     if (blocks > cap) blocks = cap;
-    k_update<<<(int)blocks, 256, 0, stream>>>(x, acc, n_voxels, lambda, ctrl, n_blocks);
-    return cudaGetLastError();
+    const cudaError_t e = launch_pdl(k_update, dim3((int)blocks), dim3(256), 0, stream, x, acc, n_voxels, lambda, ctrl, n_blocks, top_down);
+    return e != cudaSuccess ? e : cudaGetLastError();
 }
 
 // inspection: de-interleave the accumulator into Delta and c (in the voxel order of include/pct.h), and zero it

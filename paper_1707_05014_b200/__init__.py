@@ -17,6 +17,7 @@ from .binding import (  # noqa: F401
     pct_destroy,
     pct_get_image,
     pct_get_stats,
+    pct_get_tvs_state,
     pct_iterate,
     pct_iterate_carp,
     pct_measure_peaks,
@@ -25,6 +26,8 @@ from .binding import (  # noqa: F401
     pct_set_histories_host,
     pct_set_image,
     pct_set_path_model,
+    pct_set_tvs,
     pct_synchronize,
+    pct_tvs_step,
     pct_version,
 )

@@ -61,13 +61,17 @@ def lib():
         L.pct_debug_block.argtypes = [vp, i64, i64, vp, vp]
         L.pct_profile_sweep.argtypes = [vp, C.c_float, i64, C.POINTER(C.c_float)]
         L.pct_measure_peaks.argtypes = [vp, i64, C.POINTER(C.c_double)]
+        L.pct_set_tvs.argtypes = [vp, C.c_float, C.c_float, C.c_int]
+        L.pct_tvs_step.argtypes = [vp]
+        L.pct_get_tvs_state.argtypes = [vp, C.POINTER(C.c_double)]
         _lib = L
     return _lib
 
 
 EXPORTS = ("pct_create", "pct_set_histories", "pct_set_histories_host", "pct_iterate", "pct_iterate_carp", "pct_set_path_model", "pct_get_image",
            "pct_set_image", "pct_synchronize", "pct_get_stats", "pct_destroy", "pct_last_error", "pct_version",
-           "pct_debug_rows", "pct_debug_block", "pct_profile_sweep", "pct_measure_peaks")
+           "pct_debug_rows", "pct_debug_block", "pct_profile_sweep", "pct_measure_peaks", "pct_set_tvs", "pct_tvs_step",
+           "pct_get_tvs_state")
 
 
 def _ptr(a):
@@ -183,3 +187,18 @@ def pct_measure_peaks(footprint_bytes, cuda_stream=None):
     return dict(gather_random_per_s=out[0], gather_path_per_s=out[1], red_v2_random_per_s=out[2], stream_read_bytes_per_s=out[3],
                 ffma_inst_per_s=out[4], ffma2_inst_per_s=out[5], red_v2_path_per_s=out[6], footprint_bytes=int(out[7]),
                 gather_path_tiled_per_s=out[8], red_v2_path_tiled_per_s=out[9])
+
+
+def pct_set_tvs(ctx, beta0, gamma=1.0, n_halvings=4):
+    """Total-variation superiorization step before every DROP block / CARP iteration (include/pct.h); beta0 = 0: off."""
+    _check(ctx, lib().pct_set_tvs(ctx, float(beta0), float(gamma), int(n_halvings)))
+
+
+def pct_tvs_step(ctx):
+    _check(ctx, lib().pct_tvs_step(ctx))
+
+
+def pct_get_tvs_state(ctx):
+    out = (C.c_double * 6)()
+    _check(ctx, lib().pct_get_tvs_state(ctx, out))
+    return dict(beta=out[0], tv_before=out[1], tv_after=out[2], level=int(out[3]), steps=int(out[4]), accepted=int(out[5]))

@@ -82,6 +82,11 @@ struct pct_ctx {
     std::vector<WavePlan> plans;   // one per string (one for DROP)
     WaveCtrl* carp_wctrl = nullptr;
     long long carp_stride = 0;     // voxels between the images / accumulators of two strings (a multiple of four)
+    // total-variation superiorization (pct_set_tvs): off unless tvs_beta0 > 0
+    float tvs_beta0 = 0.f, tvs_gamma = 1.f;
+    int tvs_levels = 0, tvs_parity = 0;
+    float* tvs_grad = nullptr;   // n_slots floats
+    TvState* tvs_state = nullptr;
     // cached CUDA graph of kGraphPairs (accumulate, update) pairs
     cudaGraphExec_t graph = nullptr;
     float graph_lambda = 0.f;
@@ -92,6 +97,7 @@ struct pct_ctx {
 };
 
 static thread_local char g_create_err[512] = {0};
+static int tvs_step(pct_ctx* c, float* x, cudaStream_t s);
 static const int kGraphPairs = 64;
 // Upload chunks (histories): the first one is small so that the first DROP blocks start after about a
 // millisecond, the following ones double up to 2^24 (64 MB per float field) so that a 19 GB upload is
@@ -377,6 +383,8 @@ extern "C" void pct_destroy(pct_ctx* c) {
     if (c->tab) cudaFree(c->tab);
     if (c->ctrl) cudaFree(c->ctrl);
     if (c->wctrl) cudaFree(c->wctrl);
+    if (c->tvs_grad) cudaFree(c->tvs_grad);
+    if (c->tvs_state) cudaFree(c->tvs_state);
     (void)cudaGetLastError();
     delete c;
 }
@@ -662,7 +670,8 @@ extern "C" int pct_iterate(pct_ctx* c, float lambda, int64_t block_size, int n_i
     if (n_iter < 0) return fail(c, PCT_EINVAL, "pct_iterate: n_iter must be >= 0");
     if (n_iter == 0) return PCT_OK;
     DeviceGuard guard(c->device);
-    if (c->engine == 1) return iterate_wave(c, lambda, block_size, n_iter);
+    const bool tvs = c->tvs_beta0 > 0.0f;  // a step on the image that enters every block: launches go out one by one
+    if (c->engine == 1 && !tvs) return iterate_wave(c, lambda, block_size, n_iter);
     const long long n_blocks = (c->n + block_size - 1) / block_size;
     const long long pairs = n_blocks * (long long)n_iter;
     CUDA_TRY(c, cudaMemsetAsync(c->ctrl, 0, sizeof(Ctrl), c->stream));
@@ -673,7 +682,7 @@ extern "C" int pct_iterate(pct_ctx* c, float lambda, int64_t block_size, int n_i
     }
     const DropArgs a = drop_args(c, block_size, -1, 0);
     long long done = 0;
-    if (pairs >= 2 * kGraphPairs) {
+    if (pairs >= 2 * kGraphPairs && !tvs) {
         const bool reuse = c->graph && c->graph_lambda == lambda && c->graph_block == block_size && c->graph_n == c->n &&
                            c->graph_hist_key == (const void*)c->H.t_in && c->graph_order == (const void*)c->order;
         if (!reuse) {
@@ -709,6 +718,7 @@ extern "C" int pct_iterate(pct_ctx* c, float lambda, int64_t block_size, int n_i
     for (; done < pairs; ++done) {
         int rc = wait_upload(c, done < n_blocks ? (done + 1) * block_size : -1);
         if (rc == PCT_OK) rc = build_order(c, block_size, done < n_blocks ? done + 1 : n_blocks);
+        if (rc == PCT_OK && tvs) rc = tvs_step(c, c->x, c->stream);
         if (rc == PCT_OK) rc = enqueue_pair(c, a, lambda, n_blocks, c->stream);
         if (rc) return rc;
     }
@@ -769,6 +779,8 @@ extern "C" int pct_iterate_carp(pct_ctx* c, float lambda, int64_t block_size, in
         c->order_built = 1;
     }
     for (int it = 0; it < n_iter; ++it) {
+        if (c->tvs_beta0 > 0.0f)  // "In CARP, TVS is applied just once to the initial solution at the start of each iteration"
+            if (int rc = tvs_step(c, c->x, c->stream)) return rc;
         CUDA_TRY(c, cudaEventRecord(c->carp_fork, c->stream));  // x (and, the first time, the zeroed accumulators) are ready
         for (int p = 0; p < P; ++p) {
             cudaStream_t s = c->carp_stream[p];
@@ -810,6 +822,62 @@ extern "C" int pct_iterate_carp(pct_ctx* c, float lambda, int64_t block_size, in
         if (c->engine == 1)  // pct_get_stats: the counters of the strings' sweeps, added up
             CUDA_TRY(c, launch_sum_stats(c->wctrl, c->carp_wctrl, P, c->stream));
     }
+    return PCT_OK;
+}
+
+// ---- total-variation superiorization (R31) ----------------------------------------------
+
+static int tvs_step(pct_ctx* c, float* x, cudaStream_t s) {
+    CUDA_TRY(c, launch_tvs_step(x, c->tvs_grad, c->g, c->n_slots, c->tvs_state, c->tvs_parity, c->tvs_levels, c->tvs_gamma, c->sm_count, s));
+    c->tvs_parity ^= 1;
+    return PCT_OK;
+}
+
+extern "C" int pct_set_tvs(pct_ctx* c, float beta0, float gamma, int n_halvings) {
+    if (!c) return PCT_EINVAL;
+    if (!(beta0 >= 0.0f) || !isfinite(beta0)) return fail(c, PCT_EINVAL, "pct_set_tvs: beta0 must be >= 0 (0 switches the step off)");
+    DeviceGuard guard(c->device);
+    if (beta0 == 0.0f) {
+        c->tvs_beta0 = 0.f;
+        return PCT_OK;
+    }
+    if (!(gamma > 0.0f) || !(gamma <= 1.0f)) return fail(c, PCT_EINVAL, "pct_set_tvs: gamma must be in (0, 1]");
+    if (n_halvings < 1 || n_halvings > kTvMaxLevels) return fail(c, PCT_EINVAL, "pct_set_tvs: n_halvings must be in [1, 8]");
+    if (!c->tvs_grad) CUDA_TRY(c, cudaMalloc(&c->tvs_grad, sizeof(float) * c->n_slots));
+    if (!c->tvs_state) CUDA_TRY(c, cudaMalloc(&c->tvs_state, sizeof(TvState)));
+    TvState init{};
+    init.beta[0] = init.beta[1] = beta0;
+    init.beta_used = beta0;
+    init.level = -1;
+    CUDA_TRY(c, cudaMemcpyAsync(c->tvs_state, &init, sizeof(init), cudaMemcpyHostToDevice, c->stream));
+    CUDA_TRY(c, cudaStreamSynchronize(c->stream));  // (init lives on this stack frame)
+    c->tvs_beta0 = beta0;
+    c->tvs_gamma = gamma;
+    c->tvs_levels = n_halvings;
+    c->tvs_parity = 0;
+    return PCT_OK;
+}
+
+extern "C" int pct_tvs_step(pct_ctx* c) {
+    if (!c) return PCT_EINVAL;
+    if (!(c->tvs_beta0 > 0.0f)) return fail(c, PCT_ESTATE, "pct_tvs_step: the step is off (pct_set_tvs)");
+    DeviceGuard guard(c->device);
+    return tvs_step(c, c->x, c->stream);
+}
+
+extern "C" int pct_get_tvs_state(pct_ctx* c, double out[6]) {
+    if (!c || !out) return PCT_EINVAL;
+    if (!c->tvs_state) return fail(c, PCT_ESTATE, "pct_get_tvs_state: pct_set_tvs was never called");
+    DeviceGuard guard(c->device);
+    TvState h;
+    CUDA_TRY(c, cudaMemcpyAsync(&h, c->tvs_state, sizeof(h), cudaMemcpyDeviceToHost, c->stream));
+    CUDA_TRY(c, cudaStreamSynchronize(c->stream));
+    out[0] = (double)h.beta[c->tvs_parity];  // the step size the next step starts from
+    out[1] = h.tv_before;
+    out[2] = h.tv_after;
+    out[3] = (double)h.level;
+    out[4] = (double)h.steps;
+    out[5] = (double)h.accepted;
     return PCT_OK;
 }
 

@@ -122,4 +122,18 @@ cudaError_t launch_wave(const WaveArgs& a, int grid, cudaStream_t stream);
 cudaError_t launch_plan_blocks(const HistPtrs& H, const Geom& g, long long n, long long block_size, long long first_block,
                                long long n_blocks, const WaveShape& shp, uint32_t* plan, int* need, cudaStream_t stream);
 
+// ---- total-variation superiorization (pct_tvs.cu) ---------------------------------------------------------------
+constexpr int kTvMaxLevels = 8;
+struct TvState {
+    double tvx, g2;              // TV(x) and ||grad TV(x)||^2 of the step in progress
+    double tvz[kTvMaxLevels];    // TV(x + beta 2^-l v)
+    double tv_before, tv_after;  // of the last completed step
+    float beta[2];               // beta[parity]: step size of the step in progress; the other slot receives the next one
+    float beta_used;             // step of the last completed step (beta 2^-level, or beta 2^-n_half if none was accepted)
+    int level;                   // level accepted by the last step, -1: none
+    unsigned int steps, accepted;
+};
+cudaError_t launch_tvs_step(float* x, float* grad, const Geom& g, long long n_slots, TvState* st, int parity, int n_half, float gamma,
+                            int sms, cudaStream_t stream);
+
 }  // namespace pct

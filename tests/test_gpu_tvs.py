@@ -1,0 +1,117 @@
+"""TVS on the GPU (pct_set_tvs / pct_tvs_step, R31) against the fp64 oracle (oracle/tvs.py).
+
+A single step: the accepted level is the oracle's (an integer decided by comparing sums: both sides compare TV(z) with
+TV(x), the library on fp64 sums of fp32 terms; the cases are checked to be far from a tie), the image within 1e-5
+relative L2 of the oracle's step, TV before / after within 1e-6 relative.  Then DROP with a step before every block
+and CARP with a step before every iteration, image per iteration within the DROP tolerances."""
+import numpy as np
+import pytest
+
+import synth
+from helpers import oracle_geom, to_device
+from oracle import tvs
+
+pytestmark = pytest.mark.gpu
+
+
+def _ctx(pct, torch, nx, ny, nz, h=1.0):
+    r = 0.5 * h * min(nx, ny)
+    return pct.pct_create(nx, ny, nz, h, -r - 10.0, r + 10.0, torch.cuda.current_stream().cuda_stream)
+
+
+@pytest.mark.parametrize("shape,beta,levels", [((64, 64, 8), 2.0, 4), ((45, 71, 5), 0.5, 3), ((128, 128, 32), 500.0, 8), ((16, 16, 1), 0.3, 2)])
+def test_single_steps_against_the_oracle(shape, beta, levels):
+    import torch
+
+    import paper_1707_05014_b200 as pct
+
+    nx, ny, nz = shape
+    M = nx * ny * nz
+    rng = np.random.default_rng(nx * 7 + nz)
+    k, j, i = np.meshgrid(np.arange(nz), np.arange(ny), np.arange(nx), indexing="ij")
+    disc = (((i - nx / 2) ** 2 + (j - ny / 2) ** 2) < (0.35 * min(nx, ny)) ** 2).astype(np.float64)
+    x = (disc * 1.04 + rng.normal(0, 0.03, disc.shape)).astype(np.float32).reshape(-1)
+    ctx = _ctx(pct, torch, nx, ny, nz)
+    out = np.zeros(M, dtype=np.float32)
+    try:
+        pct.pct_set_image(ctx, x, M)
+        with pytest.raises(pct.PctError):
+            pct.pct_tvs_step(ctx)  # off by default
+        for bad in ((-1.0, 0.5, 3), (1.0, 0.0, 3), (1.0, 1.5, 3), (1.0, 0.5, 0), (1.0, 0.5, 9)):
+            with pytest.raises(pct.PctError):
+                pct.pct_set_tvs(ctx, *bad)
+        pct.pct_set_tvs(ctx, beta, 0.7, levels)
+        xr = x.astype(np.float64)
+        b = beta
+        accepted = 0
+        for step in range(4):
+            pct.pct_tvs_step(ctx)
+            pct.pct_get_image(ctx, out, M)
+            st = pct.pct_get_tvs_state(ctx)
+            xr_new, info = tvs.tvs_step(xr, shape, b, levels)
+            # the decision is not a near-tie on the oracle's side
+            tried = info["tv_tried"]
+            assert all(abs(t - info["tv_before"]) > 1e-6 * info["tv_before"] for t in tried), tried
+            assert st["level"] == info["level"], (step, st, info)
+            assert st["tv_before"] == pytest.approx(info["tv_before"], rel=1e-6)
+            assert st["tv_after"] == pytest.approx(info["tv_after"], rel=1e-6)
+            assert st["beta"] == pytest.approx(0.7 * info["beta_used"], rel=1e-6)
+            assert st["steps"] == step + 1
+            g = out.astype(np.float64)
+            assert np.linalg.norm(g - xr_new) <= 1e-5 * np.linalg.norm(xr_new), step
+            assert np.abs(g - xr_new).max() <= 1e-5
+            if info["level"] >= 0:  # the step has length beta_used in the 2-norm
+                assert np.linalg.norm(g - xr) == pytest.approx(info["beta_used"], rel=1e-3)
+                accepted += 1
+            xr, b = xr_new, 0.7 * info["beta_used"]
+        assert accepted >= 2 and st["accepted"] == accepted
+        pct.pct_set_tvs(ctx, 0.0, 1.0, 1)  # off again
+        with pytest.raises(pct.PctError):
+            pct.pct_tvs_step(ctx)
+    finally:
+        pct.pct_destroy(ctx)
+
+
+def test_drop_and_carp_with_tvs_against_the_oracle(oracle_mod):
+    import torch
+
+    import paper_1707_05014_b200 as pct
+
+    oracle = oracle_mod
+    cfg = synth.config(0)
+    n, B, lam = 12_000, 1000, 0.5
+    H = synth.generate_numpy(cfg, n)
+    geom = oracle_geom(oracle, cfg)
+    hs = oracle.Histories(H)
+    D = to_device(H)
+    M = cfg.n_voxels
+    shape = (cfg.nx, cfg.ny, cfg.nz)
+    ctx = pct.pct_create(cfg.nx, cfg.ny, cfg.nz, cfg.h, cfg.u_in, cfg.u_out, torch.cuda.current_stream().cuda_stream)
+    out = np.zeros(M, dtype=np.float32)
+    try:
+        pct.pct_set_histories(ctx, n, D)
+        pct.pct_set_tvs(ctx, 0.4, 0.98, 4)
+        x_ref, beta = np.zeros(M), 0.4
+        for it in range(3):
+            pct.pct_iterate(ctx, lam, B, 1)
+            pct.pct_get_image(ctx, out, M)
+            x_ref, beta, infos = tvs.drop_iterate_tvs(oracle, geom, hs, lam, B, 1, x_ref, beta, 0.98, 4)
+            g = out.astype(np.float64)
+            assert np.linalg.norm(g - x_ref) <= 1e-4 * np.linalg.norm(x_ref), it
+            st = pct.pct_get_tvs_state(ctx)
+            assert st["steps"] == 12 * (it + 1) and st["beta"] == pytest.approx(beta, rel=1e-5)
+            assert st["level"] == infos[-1]["level"]
+        assert np.abs(g - x_ref).max() <= 1e-3
+        # the same three sweeps without the step are rougher (the step smooths: PAPER.md:113)
+        plain, _ = oracle.drop_iterate(geom, hs, lam, B, 3, np.zeros(M))
+        assert tvs.tv(g, shape) < tvs.tv(plain, shape)
+        # CARP: one step per iteration on the common start
+        for it in range(2):
+            pct.pct_iterate_carp(ctx, lam, B, 1, 3)
+            pct.pct_get_image(ctx, out, M)
+            x_ref, beta, infos = tvs.carp_iterate_tvs(oracle, geom, hs, lam, B, 1, 3, x_ref, beta, 0.98, 4)
+            g = out.astype(np.float64)
+            assert np.linalg.norm(g - x_ref) <= 1e-4 * np.linalg.norm(x_ref), it
+        assert pct.pct_get_tvs_state(ctx)["steps"] == 38
+    finally:
+        pct.pct_destroy(ctx)

@@ -3,7 +3,7 @@ and per-cent error of the RSP inside every insert -- the synthetic counterpart o
 (PAPER.md:111-126: "mean RSP value and standard deviation for a region of interest within each insert").
 Analysis of the OUTPUT only; none of the method's arithmetic.
 
-    python -m synth.roi --config 1 [--iterations 6] [--carp-strings 4] [--histories 1e7]
+    python -m synth.roi --config 1 [--iterations 6] [--carp-strings 4] [--histories 1e7] [--tvs 0.5 0.9995 4]
 
 runs the reconstruction on cuda:0 through the C ABI and prints the table (markdown)."""
 import argparse
@@ -49,7 +49,7 @@ def markdown(rows):
     return "\n".join(out)
 
 
-def reconstruct(cfg, n, n_iter, carp_strings=0, spline=False):
+def reconstruct(cfg, n, n_iter, carp_strings=0, spline=False, tvs=None):
     """The reconstruction of cfg's first n histories on cuda:0 through the C ABI -> image (numpy float32)."""
     import torch
 
@@ -62,6 +62,8 @@ def reconstruct(cfg, n, n_iter, carp_strings=0, spline=False):
     try:
         pct.pct_set_histories(ctx, n, D)
         pct.pct_set_path_model(ctx, pct.PCT_PATH_SPLINE if spline else pct.PCT_PATH_MLP)
+        if tvs is not None:  # (beta0, gamma, n_halvings): total-variation superiorization
+            pct.pct_set_tvs(ctx, *tvs)
         if carp_strings > 0:
             pct.pct_iterate_carp(ctx, cfg.lam, cfg.block_size, n_iter, carp_strings)
         else:
@@ -80,18 +82,23 @@ def main():
     ap.add_argument("--iterations", type=int, default=None)
     ap.add_argument("--carp-strings", type=int, default=0)
     ap.add_argument("--spline", action="store_true", help="cubic-spline path model instead of the most-likely path")
+    ap.add_argument("--tvs", type=float, nargs=3, default=None, metavar=("BETA0", "GAMMA", "HALVINGS"),
+                    help="total-variation superiorization step before every DROP block / CARP iteration (PAPER.md:113)")
     ap.add_argument("--json", action="store_true")
     a = ap.parse_args()
     cfg = config(a.config)
     n = cfg.n if a.histories is None else int(a.histories)
     it = cfg.n_iter if a.iterations is None else a.iterations
-    img = reconstruct(cfg, n, it, a.carp_strings, a.spline)
+    tvs = None if a.tvs is None else (a.tvs[0], a.tvs[1], int(a.tvs[2]))
+    img = reconstruct(cfg, n, it, a.carp_strings, a.spline, tvs)
     rows = roi_table(cfg, img)
     truth = rsp_volume(cfg)
     hull = truth > 10 * AIR
     rms = float(np.sqrt(np.mean((img[hull] - truth[hull]) ** 2)))
     head = "%s, %d histories, %d iterations, %s, lambda %.3g, block %d; RMS error inside the object %.4f" % (
         cfg.workload, n, it, ("CARP with %d strings" % a.carp_strings if a.carp_strings else "DROP") + (", spline path" if a.spline else ", most-likely path"), cfg.lam, cfg.block_size, rms)
+    if tvs is not None:
+        head += "; TVS beta0 %g, gamma %g, %d halvings" % tvs
     if a.json:
         print(json.dumps(dict(run=head, rows=rows, rms=rms)))
     else:

@@ -26,4 +26,6 @@ from .binding import (  # noqa: F401
     set_path_model,
     sigma1_table,
     sigma_f64,
+    xyz_to_beam_f32,
+    xyz_to_beam_f64,
 )

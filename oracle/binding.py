@@ -284,3 +284,29 @@ def get_path_model():
 
 def num_threads():
     return int(lib().orc_num_threads())
+
+
+def xyz_to_beam_f32(u_pl, x, y, z, tht, thv, proj, proj_cos, proj_sin):
+    """Object-frame tracker hits -> (t, v) at the tracker plane u_pl, fp32 rule (R32)."""
+    f32 = lambda a: np.ascontiguousarray(a, dtype=np.float32)
+    x, y, z, tht, thv, pc, ps = (f32(a) for a in (x, y, z, tht, thv, proj_cos, proj_sin))
+    proj = np.ascontiguousarray(proj, dtype=np.uint16)
+    n = x.shape[0]
+    t = np.zeros(n, dtype=np.float32)
+    v = np.zeros(n, dtype=np.float32)
+    fp = lambda a: a.ctypes.data_as(_FP)
+    L = lib()
+    L.orc_xyz_to_beam_f32.argtypes = [C.c_float, C.c_int] + [_FP] * 5 + [C.POINTER(C.c_uint16), _FP, _FP, C.c_int, _FP, _FP]
+    L.orc_xyz_to_beam_f32.restype = None
+    L.orc_xyz_to_beam_f32(float(u_pl), n, fp(x), fp(y), fp(z), fp(tht), fp(thv), proj.ctypes.data_as(C.POINTER(C.c_uint16)),
+                          fp(pc), fp(ps), int(pc.shape[0]), fp(t), fp(v))
+    return t, v
+
+
+def xyz_to_beam_f64(u_pl, x, y, z, tht, thv, cs, sn):
+    out = np.zeros(2)
+    L = lib()
+    L.orc_xyz_to_beam_f64.argtypes = [C.c_double] * 8 + [C.POINTER(C.c_double)]
+    L.orc_xyz_to_beam_f64.restype = None
+    L.orc_xyz_to_beam_f64(float(u_pl), float(x), float(y), float(z), float(tht), float(thv), float(cs), float(sn), _dp(out))
+    return out

@@ -732,3 +732,33 @@ int orc_num_threads(void) {
     return 1;
 #endif
 }
+
+/* ==========================================================================================
+ * Object-frame entry point (R32): a history given as tracker HITS
+ * (x, y, z) in the object frame plus its beam-frame slopes.  The hit is carried along its straight
+ * ray (air, R7) to the tracker plane of the rule:
+ *     u = fma(y, cos, -(x sin));  t = fma(x, cos, y sin)          (rotation about z by -phi, R8)
+ *     t_pl = fma(theta_t, u_pl - u, t);  v_pl = fma(theta_v, u_pl - u, z)
+ * fp32, this operation order (it feeds the rule that decides voxel indices).  *_f64: the same in
+ * double, the definition the pins check.
+ * ======================================================================================== */
+void orc_xyz_to_beam_f32(float u_pl, int n, const float *x, const float *y, const float *z, const float *tht,
+                         const float *thv, const uint16_t *proj, const float *pcos, const float *psin, int n_proj,
+                         float *t_out, float *v_out) {
+    for (int i = 0; i < n; ++i) {
+        int p = proj[i];
+        if (p >= n_proj) p = n_proj - 1; /* R24 */
+        const float cs = pcos[p], sn = psin[p];
+        const float u = fmaf(y[i], cs, -(x[i] * sn));
+        const float t = fmaf(x[i], cs, y[i] * sn);
+        const float du = u_pl - u;
+        t_out[i] = fmaf(tht[i], du, t);
+        v_out[i] = fmaf(thv[i], du, z[i]);
+    }
+}
+void orc_xyz_to_beam_f64(double u_pl, double x, double y, double z, double tht, double thv, double cs, double sn,
+                         double out[2]) {
+    const double u = -x * sn + y * cs, t = x * cs + y * sn;
+    out[0] = t + tht * (u_pl - u);
+    out[1] = z + thv * (u_pl - u);
+}

@@ -24,6 +24,7 @@ from .binding import (  # noqa: F401
     pct_profile_sweep,
     pct_set_histories,
     pct_set_histories_host,
+    pct_set_histories_xyz,
     pct_set_image,
     pct_set_path_model,
     pct_set_tvs,

@@ -24,6 +24,14 @@ class pct_histories(C.Structure):
                                                      ("proj_sin", C.c_void_p), ("n_proj", C.c_int32)]
 
 
+XYZ_FIELDS = ("entry_x", "entry_y", "entry_z", "exit_x", "exit_y", "exit_z", "entry_dt", "entry_dv", "exit_dt", "exit_dv", "wepl")
+
+
+class pct_histories_xyz(C.Structure):
+    _fields_ = [(n, C.c_void_p) for n in XYZ_FIELDS] + [("proj", C.c_void_p), ("proj_cos", C.c_void_p),
+                                                         ("proj_sin", C.c_void_p), ("n_proj", C.c_int32)]
+
+
 class PctError(RuntimeError):
     def __init__(self, code, msg):
         super().__init__("%s: %s" % (_STATUS.get(code, code), msg))
@@ -45,6 +53,7 @@ def lib():
         L.pct_create.argtypes = [C.POINTER(vp), C.c_int, C.c_int, C.c_int, C.c_float, C.c_float, C.c_float, vp]
         L.pct_set_histories.argtypes = [vp, i64, C.POINTER(pct_histories)]
         L.pct_set_histories_host.argtypes = [vp, i64, C.POINTER(pct_histories)]
+        L.pct_set_histories_xyz.argtypes = [vp, i64, C.POINTER(pct_histories_xyz)]
         L.pct_iterate.argtypes = [vp, C.c_float, i64, C.c_int]
         L.pct_iterate_carp.argtypes = [vp, C.c_float, i64, C.c_int, C.c_int]
         L.pct_set_path_model.argtypes = [vp, C.c_int]
@@ -68,7 +77,7 @@ def lib():
     return _lib
 
 
-EXPORTS = ("pct_create", "pct_set_histories", "pct_set_histories_host", "pct_iterate", "pct_iterate_carp", "pct_set_path_model", "pct_get_image",
+EXPORTS = ("pct_create", "pct_set_histories", "pct_set_histories_host", "pct_set_histories_xyz", "pct_iterate", "pct_iterate_carp", "pct_set_path_model", "pct_get_image",
            "pct_set_image", "pct_synchronize", "pct_get_stats", "pct_destroy", "pct_last_error", "pct_version",
            "pct_debug_rows", "pct_debug_block", "pct_profile_sweep", "pct_measure_peaks", "pct_set_tvs", "pct_tvs_step",
            "pct_get_tvs_state")
@@ -123,6 +132,15 @@ def pct_set_histories_host(ctx, n, arrays):
     """arrays: mapping of host arrays (numpy or CPU tensors, ideally pinned); the library copies them."""
     s, _ = _hist_struct(arrays)
     _check(ctx, lib().pct_set_histories_host(ctx, int(n), C.byref(s)))
+
+
+def pct_set_histories_xyz(ctx, n, arrays):
+    """arrays: mapping of CUDA tensors keyed as pct_histories_xyz (object-frame tracker hits + beam-frame slopes)."""
+    s = pct_histories_xyz()
+    for k in XYZ_FIELDS + ("proj", "proj_cos", "proj_sin"):
+        setattr(s, k, _ptr(arrays[k]))
+    s.n_proj = int(arrays["proj_cos"].shape[0])
+    _check(ctx, lib().pct_set_histories_xyz(ctx, int(n), C.byref(s)))
 
 
 def pct_iterate(ctx, lam, block_size, n_iter):

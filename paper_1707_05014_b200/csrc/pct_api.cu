@@ -429,6 +429,54 @@ extern "C" int pct_set_histories(pct_ctx* c, int64_t n, const pct_histories* h) 
     return PCT_OK;
 }
 
+extern "C" int pct_set_histories_xyz(pct_ctx* c, int64_t n, const pct_histories_xyz* h) {
+    if (!c) return PCT_EINVAL;
+    if (!h) return fail(c, PCT_EINVAL, "pct_set_histories_xyz: h is NULL");
+    if (n < 1 || n >= (1LL << 40)) return fail(c, PCT_EINVAL, "pct_set_histories_xyz: n must be in [1, 2^40)");
+    if (h->n_proj < 1 || h->n_proj > 65536) return fail(c, PCT_EINVAL, "pct_set_histories_xyz: n_proj must be in [1, 65536]");
+    const void* ptrs[14] = {h->entry_x, h->entry_y, h->entry_z, h->exit_x, h->exit_y, h->exit_z, h->entry_dt, h->entry_dv,
+                            h->exit_dt, h->exit_dv, h->wepl, h->proj, h->proj_cos, h->proj_sin};
+    for (int i = 0; i < 14; ++i)
+        if (!ptrs[i] || !is_device_ptr(ptrs[i])) return fail(c, PCT_EINVAL, "pct_set_histories_xyz: arrays must be device memory");
+    DeviceGuard guard(c->device);
+    release_histories(c);
+    // four owned arrays (positions at the tracker planes, each padded to 256 B); slopes, WEPL and proj stay borrowed
+    const size_t fa = ((sizeof(float) * (size_t)n + 255) / 256) * 256;
+    cudaError_t e = cudaMalloc(&c->owned_hist, 4 * fa);
+    if (e == cudaSuccess) e = cudaMalloc(&c->tables, sizeof(float) * 2 * h->n_proj);
+    if (e != cudaSuccess) {
+        release_histories(c);
+        CUDA_TRY(c, e);
+    }
+    c->owned_n = -1;  // (not a block of the host entry point: never reused by it)
+    float* d[4];
+    for (int i = 0; i < 4; ++i) d[i] = (float*)((char*)c->owned_hist + i * fa);
+    float* pc = c->tables;
+    float* ps = c->tables + h->n_proj;
+    int rc = PCT_OK;
+    auto body = [&]() -> int {
+        CUDA_TRY(c, cudaMemcpyAsync(pc, h->proj_cos, sizeof(float) * h->n_proj, cudaMemcpyDeviceToDevice, c->stream));
+        CUDA_TRY(c, cudaMemcpyAsync(ps, h->proj_sin, sizeof(float) * h->n_proj, cudaMemcpyDeviceToDevice, c->stream));
+        CUDA_TRY(c, launch_xyz_to_beam(c->g.u_in, n, h->entry_x, h->entry_y, h->entry_z, h->entry_dt, h->entry_dv, h->proj, pc, ps, h->n_proj,
+                                       d[0], d[1], c->stream));
+        CUDA_TRY(c, launch_xyz_to_beam(c->g.u_out, n, h->exit_x, h->exit_y, h->exit_z, h->exit_dt, h->exit_dv, h->proj, pc, ps, h->n_proj,
+                                       d[2], d[3], c->stream));
+        return PCT_OK;
+    };
+    rc = body();
+    if (rc != PCT_OK) {
+        char keep[512];
+        memcpy(keep, c->err, 512);
+        release_histories(c);
+        memcpy(c->err, keep, 512);
+        return rc;
+    }
+    c->H = HistPtrs{d[0], d[1], d[2], d[3], h->entry_dt, h->entry_dv, h->exit_dt, h->exit_dv, h->wepl, h->proj, pc, ps, h->n_proj};
+    c->n = n;
+    c->have_hist = true;
+    return PCT_OK;
+}
+
 static int set_histories_host_impl(pct_ctx* c, int64_t n, const pct_histories* h);
 
 extern "C" int pct_set_histories_host(pct_ctx* c, int64_t n, const pct_histories* h) {

@@ -57,6 +57,9 @@ cudaError_t launch_drop_block(const DropArgs& a, int grid, cudaStream_t stream);
 cudaError_t launch_update(float* x, float2* acc, long long n_voxels, float lambda, Ctrl* ctrl,
                           long long n_blocks, bool top_down, cudaStream_t stream);
 cudaError_t launch_split_acc(float2* acc, float* delta, float* cnt, const Geom& g, cudaStream_t stream);
+cudaError_t launch_xyz_to_beam(float u_pl, long long n, const float* x, const float* y, const float* z, const float* tht, const float* thv,
+                               const uint16_t* proj, const float* pcos, const float* psin, int n_proj, float* t_out, float* v_out,
+                               cudaStream_t stream);
 cudaError_t launch_image_io(float* x, float* ext, const Geom& g, bool to_storage, cudaStream_t stream);
 cudaError_t launch_rows(const RowsArgs& a, cudaStream_t stream);
 cudaError_t launch_mean(float* x, const float* xs, int n_strings, long long n_voxels, long long pitch, cudaStream_t stream);

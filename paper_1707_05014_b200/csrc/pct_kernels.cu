@@ -547,6 +547,37 @@ cudaError_t launch_order_blocks(const HistPtrs& H, const Geom& g, long long n, l
     return cudaGetLastError();
 }
 
+// Object-frame entry point (include/pct.h pct_set_histories_xyz; R32): tracker hits (x, y, z) in the object
+// frame are carried along their straight rays to the tracker planes of the rule.  fp32, this operation order:
+//   u = fma(y, cos, -(x sin));  t = fma(x, cos, y sin);  t_pl = fma(theta_t, u_pl - u, t);  v_pl = fma(theta_v, u_pl - u, z)
+__global__ void __launch_bounds__(256) k_xyz_to_beam(float u_pl, long long n, const float* __restrict__ x, const float* __restrict__ y,
+                                                     const float* __restrict__ z, const float* __restrict__ tht, const float* __restrict__ thv,
+                                                     const uint16_t* __restrict__ proj, const float* __restrict__ pcos,
+                                                     const float* __restrict__ psin, int n_proj, float* __restrict__ t_out,
+                                                     float* __restrict__ v_out) {
+    const long long stride = (long long)gridDim.x * blockDim.x;
+    for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += stride) {
+        int p = (int)proj[i];
+        p = p < n_proj ? p : n_proj - 1;
+        const float cs = __ldg(pcos + p), sn = __ldg(psin + p);
+        const float u = __fmaf_rn(y[i], cs, -__fmul_rn(x[i], sn));
+        const float t = __fmaf_rn(x[i], cs, __fmul_rn(y[i], sn));
+        const float du = __fsub_rn(u_pl, u);
+        t_out[i] = __fmaf_rn(tht[i], du, t);
+        v_out[i] = __fmaf_rn(thv[i], du, z[i]);
+    }
+}
+
+cudaError_t launch_xyz_to_beam(float u_pl, long long n, const float* x, const float* y, const float* z, const float* tht, const float* thv,
+                               const uint16_t* proj, const float* pcos, const float* psin, int n_proj, float* t_out, float* v_out,
+                               cudaStream_t stream) {
+    long long blocks = (n + 255) / 256;
+    const long long cap = (long long)sm_count() * 16;
+    if (blocks > cap) blocks = cap;
+    k_xyz_to_beam<<<(int)blocks, 256, 0, stream>>>(u_pl, n, x, y, z, tht, thv, proj, pcos, psin, n_proj, t_out, v_out);
+    return cudaGetLastError();
+}
+
 // CARP (R29): the new solution is the arithmetic mean of the P string solutions, voxel by
 // voxel; summed in the order of the strings (deterministic).  xs = P images of n voxels, back to back.
 // xs = P images, `pitch` voxels apart.

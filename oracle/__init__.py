@@ -15,6 +15,7 @@ from .binding import (  # noqa: F401
     carp_iterate,
     drop_iterate,
     get_path_model,
+    get_substeps,
     lib,
     mlp_chi2_f64,
     mlp_matrix_f64,
@@ -24,6 +25,7 @@ from .binding import (  # noqa: F401
     rule_log,
     scatter_f,
     set_path_model,
+    set_substeps,
     sigma1_table,
     sigma_f64,
     xyz_to_beam_f32,

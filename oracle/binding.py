@@ -192,7 +192,7 @@ def sigma1_table(h, kmax):
 
 def path_f64(geom, hist):
     """T64 nodes (n,3) float64 in the object frame and hull tuple (u0,t0,v0,u2,t2,v2,L); (None, None) if skipped."""
-    n = geom.nmin + 3
+    n = get_substeps() * geom.nmin + 3
     nodes = np.zeros((n, 3))
     hull = np.zeros(7)
     g, h = geom.c(), hist
@@ -207,8 +207,8 @@ def path_f64(geom, hist):
 def row_f32(geom, hist, table=None):
     """One history through the fp32 rule.  Returns dict(nnz,row_idx,row_len,seg_idx,seg_len,nodes,coefs)."""
     if table is None:
-        table = sigma1_table(geom.h, geom.nmin)
-    ms = geom.nmin + 2
+        table = sigma1_table(geom.h / get_substeps(), get_substeps() * geom.nmin)
+    ms = get_substeps() * geom.nmin + 2
     row_idx = np.zeros(ms, dtype=np.int32)
     row_len = np.zeros(ms, dtype=np.float32)
     seg_idx = np.zeros(ms, dtype=np.int32)
@@ -310,3 +310,12 @@ def xyz_to_beam_f64(u_pl, x, y, z, tht, thv, cs, sn):
     L.orc_xyz_to_beam_f64.restype = None
     L.orc_xyz_to_beam_f64(float(u_pl), float(x), float(y), float(z), float(tht), float(thv), float(cs), float(sn), _dp(out))
     return out
+
+
+def set_substeps(n):
+    """1: depth step = one voxel edge (R9, default); 2: half-voxel step (R33).  Process-wide, like the path model."""
+    lib().orc_set_substeps(int(n))
+
+
+def get_substeps():
+    return int(lib().orc_get_substeps())

@@ -238,6 +238,16 @@ static int g_path_model = 0;
 void orc_set_path_model(int m) { g_path_model = m == 1 ? 1 : 0; }
 int orc_get_path_model(void) { return g_path_model; }
 
+/* Depth step of the path (R33).  1: one voxel edge h (R9, the graded path).
+ * 2: the HALF-VOXEL step h/2 -- nodes at depth k h/2, K = floor((L - eps) / (h/2)) capped at 2 min(nx, ny), the
+ * Sigma1^-1 table at s = k h/2; everything else (hull, coefficients, voxel rule, merge, DROP) unchanged. */
+static int g_substeps = 1;
+void orc_set_substeps(int n) { g_substeps = n == 2 ? 2 : 1; }
+int orc_get_substeps(void) { return g_substeps; }
+static float r32_step(const orc_geom *g) { return g_substeps == 2 ? 0.5f * g->h : g->h; }
+static int orc_kmax(const orc_geom *g) { return g_substeps * (g->nx < g->ny ? g->nx : g->ny); }
+float orc_step(const orc_geom *g) { return r32_step(g); }
+
 static double spline_f64(double s1, double L, const double y0[2], const double y2[2]) {
     const double sigma = (y2[0] - y0[0]) / L, a0 = y0[1] - sigma, a2 = y2[1] - sigma, tau = s1 / L;
     return y0[0] + sigma * s1 + L * tau * (1.0 - tau) * (1.0 - tau) * a0 - L * tau * tau * (1.0 - tau) * a2;
@@ -265,7 +275,8 @@ int orc_path_f64(const orc_geom *g, const orc_hist *hh, int max_nodes, double *n
         hullout[0] = u0; hullout[1] = t0; hullout[2] = v0;
         hullout[3] = u2; hullout[4] = t2; hullout[5] = v2; hullout[6] = L;
     }
-    int K = (int)floor((L - ORC_EPS) / h);
+    const double step = h / (double)g_substeps;
+    int K = (int)floor((L - ORC_EPS) / step);
     if (K + 2 > max_nodes) return -(K + 2);
     double cs = hh->cs, sn = hh->sn;
     for (int k = 0; k <= K + 1; ++k) {
@@ -273,7 +284,7 @@ int orc_path_f64(const orc_geom *g, const orc_hist *hh, int max_nodes, double *n
         if (k == 0) { t = t0; u = u0; v = v0; }
         else if (k == K + 1) { t = t2; u = u2; v = v2; }
         else {
-            double s1 = k * h;
+            double s1 = k * step;
             double yt0[2] = {t0, th0}, yt2[2] = {t2, th2}, yv0[2] = {v0, ph0}, yv2[2] = {v2, ph2};
             double y[2];
             if (g_path_model == 1) {
@@ -415,8 +426,9 @@ static int r32_setup(const orc_geom *g, const orc_hist *hh, r32_state *st) {
         st->qa[j] = q[j] * (1.0f / (float)(j + 3));
     }
     /* step 4 node count */
-    int K = (int)floorf((L - REPS) * inv_h);
-    if (K > nmin) K = nmin;
+    const float inv_step = 1.0f / r32_step(g);
+    int K = (int)floorf((L - REPS) * inv_step);
+    if (K > orc_kmax(g)) K = orc_kmax(g);
     st->K = K;
     return 1;
 }
@@ -473,7 +485,7 @@ static void r32_node(const orc_geom *g, const orc_hist *hh, const r32_state *st,
     else if (k == st->K + 1) { t = st->t2; u = st->u2; v = st->v2; }
     else {
         float s1, c0, c2;
-        r32_coef(st, g->h, k, p11t, p12t, p22t, &s1, &c0, &c2);
+        r32_coef(st, r32_step(g), k, p11t, p12t, p22t, &s1, &c0, &c2);
         t = fmaf(c2, st->al2, fmaf(c0, st->al0, fmaf(st->sig_t, s1, st->t0)));
         v = fmaf(c2, st->be2, fmaf(c0, st->be0, fmaf(st->sig_v, s1, st->v0)));
         u = st->u0 + s1;
@@ -512,7 +524,7 @@ int orc_row_f32(const orc_geom *g, const orc_hist *hh, const float *p11t, const 
         if (nodes) memcpy(nodes + 3 * (k + 1), cur, 12);
         if (coefs) {
             float s1 = 0, c0 = 0, c2 = 0;
-            if (k + 1 <= K) r32_coef(&st, g->h, k + 1, p11t, p12t, p22t, &s1, &c0, &c2);
+            if (k + 1 <= K) r32_coef(&st, r32_step(g), k + 1, p11t, p12t, p22t, &s1, &c0, &c2);
             coefs[2 * (k + 1)] = c0;
             coefs[2 * (k + 1) + 1] = c2;
         }
@@ -594,7 +606,7 @@ static int row_f64(const orc_geom *g, const orc_histories *H, int64_t i, const f
 int orc_block_accumulate(const orc_geom *g, const orc_histories *H, int64_t first, int64_t count,
                          const double *x, double *delta, int32_t *cnt, int64_t *stats,
                          int nthreads) {
-    const int nmin = g->nx < g->ny ? g->nx : g->ny;
+    const int nmin = orc_kmax(g); /* (most interior nodes a path can have) */
     const int max_seg = nmin + 2;
     const int64_t M = (int64_t)g->nx * g->ny * g->nz;
     float *p11t = (float *)malloc(sizeof(float) * (nmin + 1));
@@ -605,7 +617,7 @@ int orc_block_accumulate(const orc_geom *g, const orc_histories *H, int64_t firs
     int32_t *rnnz = (int32_t *)malloc(sizeof(int32_t) * (size_t)count);
     double *res = (double *)malloc(sizeof(double) * (size_t)count);
     if (!p11t || !p12t || !p22t || !ridx || !rlen || !rnnz || !res) return -2;
-    orc_sigma1_table(g->h, nmin, p11t, p12t, p22t);
+    orc_sigma1_table(r32_step(g), nmin, p11t, p12t, p22t);
     int64_t nseg_total = 0;
 #ifdef _OPENMP
     if (nthreads > 0) omp_set_num_threads(nthreads);

@@ -27,6 +27,7 @@ from .binding import (  # noqa: F401
     pct_set_histories_xyz,
     pct_set_image,
     pct_set_path_model,
+    pct_set_step,
     pct_set_tvs,
     pct_synchronize,
     pct_tvs_step,

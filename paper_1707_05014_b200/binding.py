@@ -71,6 +71,7 @@ def lib():
         L.pct_profile_sweep.argtypes = [vp, C.c_float, i64, C.POINTER(C.c_float)]
         L.pct_measure_peaks.argtypes = [vp, i64, C.POINTER(C.c_double)]
         L.pct_set_tvs.argtypes = [vp, C.c_float, C.c_float, C.c_int]
+        L.pct_set_step.argtypes = [vp, C.c_int]
         L.pct_tvs_step.argtypes = [vp]
         L.pct_get_tvs_state.argtypes = [vp, C.POINTER(C.c_double)]
         _lib = L
@@ -79,7 +80,7 @@ def lib():
 
 EXPORTS = ("pct_create", "pct_set_histories", "pct_set_histories_host", "pct_set_histories_xyz", "pct_iterate", "pct_iterate_carp", "pct_set_path_model", "pct_get_image",
            "pct_set_image", "pct_synchronize", "pct_get_stats", "pct_destroy", "pct_last_error", "pct_version",
-           "pct_debug_rows", "pct_debug_block", "pct_profile_sweep", "pct_measure_peaks", "pct_set_tvs", "pct_tvs_step",
+           "pct_debug_rows", "pct_debug_block", "pct_profile_sweep", "pct_measure_peaks", "pct_set_tvs", "pct_tvs_step", "pct_set_step",
            "pct_get_tvs_state")
 
 
@@ -220,3 +221,8 @@ def pct_get_tvs_state(ctx):
     out = (C.c_double * 6)()
     _check(ctx, lib().pct_get_tvs_state(ctx, out))
     return dict(beta=out[0], tv_before=out[1], tv_after=out[2], level=int(out[3]), steps=int(out[4]), accepted=int(out[5]))
+
+
+def pct_set_step(ctx, substeps):
+    """Depth step of the path: 1 = one voxel edge (default), 2 = half a voxel edge (include/pct.h)."""
+    _check(ctx, lib().pct_set_step(ctx, int(substeps)))

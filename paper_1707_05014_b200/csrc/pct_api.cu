@@ -286,6 +286,8 @@ extern "C" int pct_create(pct_ctx** out, int nx, int ny, int nz, float h, float 
     g.u_in = u_in; g.u_out = u_out;
     g.hx = 0.5f * (float)nx; g.hy = 0.5f * (float)ny; g.hz = 0.5f * (float)nz;
     g.fnx = (float)nx; g.fny = (float)ny; g.fnz = (float)nz;
+    g.inv_step = g.inv_h;  // (pct_set_step: one voxel edge per node by default, R9)
+    g.kmax = nmin;
     if (!(u_in <= -R) || !(u_out >= R) || !isfinite(u_in) || !isfinite(u_out))
         return fail(nullptr, PCT_EINVAL, "pct_create: tracker planes must lie outside the hull (u_in <= -R_h, u_out >= R_h)");
     pct_ctx* c = new (std::nothrow) pct_ctx;
@@ -309,7 +311,7 @@ extern "C" int pct_create(pct_ctx** out, int nx, int ny, int nz, float h, float 
         CUDA_TRY(nullptr, cudaMalloc(&c->x, sizeof(float) * c->n_slots));
         CUDA_TRY(nullptr, cudaMalloc(&c->acc, sizeof(float2) * c->n_slots));
         CUDA_TRY(nullptr, cudaMalloc(&c->io_buf, sizeof(float) * c->n_voxels));
-        CUDA_TRY(nullptr, cudaMalloc(&c->tab, sizeof(float4) * (nmin + 1)));
+        CUDA_TRY(nullptr, cudaMalloc(&c->tab, sizeof(float4) * (2 * nmin + 1)));  // (room for the half-voxel step)
         CUDA_TRY(nullptr, cudaMalloc(&c->ctrl, sizeof(Ctrl)));
         CUDA_TRY(nullptr, cudaMemsetAsync(c->x, 0, sizeof(float) * c->n_slots, c->stream));
         CUDA_TRY(nullptr, cudaMemsetAsync(c->acc, 0, sizeof(float2) * c->n_slots, c->stream));
@@ -929,6 +931,34 @@ extern "C" int pct_get_tvs_state(pct_ctx* c, double out[6]) {
     return PCT_OK;
 }
 
+// The depth step of the path (R9, R33): the Sigma1^-1 table at the new node depths, the node count, the
+// shared memory of the walk kernels.
+extern "C" int pct_set_step(pct_ctx* c, int substeps) {
+    if (!c) return PCT_EINVAL;
+    if (substeps != 1 && substeps != 2) return fail(c, PCT_EINVAL, "pct_set_step: substeps must be 1 (voxel edge) or 2 (half a voxel edge)");
+    DeviceGuard guard(c->device);
+    const int kmax = substeps * c->g.nmin;
+    if (kmax == c->g.kmax) return PCT_OK;
+    int smem_max = 0;
+    CUDA_TRY(c, cudaDeviceGetAttribute(&smem_max, cudaDevAttrMaxSharedMemoryPerBlockOptin, c->device));
+    if (((kmax + 32) >> 5) > 64 || wave_smem_need(kmax) > (size_t)smem_max)
+        return fail(c, PCT_EINVAL, "pct_set_step: the grid is too wide for the half-voxel step (row buffer does not fit shared memory)");
+    const float step = substeps == 2 ? 0.5f * c->g.h : c->g.h;
+    float4* tab = (float4*)malloc(sizeof(float4) * (kmax + 1));
+    if (!tab) return fail(c, PCT_ENOMEM, "pct_set_step: out of host memory");
+    sigma1_inverse_table(step, kmax, tab);
+    CUDA_TRY(c, cudaStreamSynchronize(c->stream));  // (kernels in flight still read the old table)
+    cudaError_t e = cudaMemcpy(c->tab, tab, sizeof(float4) * (kmax + 1), cudaMemcpyHostToDevice);
+    free(tab);
+    CUDA_TRY(c, e);
+    CUDA_TRY(c, drop_configure(kmax, &c->drop_grid));
+    CUDA_TRY(c, wave_configure(kmax, &c->wave_grid));
+    c->g.kmax = kmax;
+    c->g.inv_step = 1.0f / step;
+    drop_graph(c);  // the cached graph holds the old geometry
+    return PCT_OK;
+}
+
 extern "C" int pct_set_path_model(pct_ctx* c, int model) {
     if (!c) return PCT_EINVAL;
     if (model != PCT_PATH_MLP && model != PCT_PATH_SPLINE) return fail(c, PCT_EINVAL, "pct_set_path_model: unknown model");
@@ -989,7 +1019,7 @@ extern "C" int pct_debug_rows(pct_ctx* c, int64_t first, int64_t count, int32_t 
     if (!c) return PCT_EINVAL;
     if (!c->have_hist) return fail(c, PCT_ESTATE, "pct_debug_rows: no histories set");
     if (first < 0 || count < 1 || first + count > c->n) return fail(c, PCT_EINVAL, "pct_debug_rows: range outside the histories");
-    if (max_seg < c->g.nmin + 2) return fail(c, PCT_EINVAL, "pct_debug_rows: max_seg must be >= min(nx,ny)+2");
+    if (max_seg < c->g.kmax + 2) return fail(c, PCT_EINVAL, "pct_debug_rows: max_seg must be >= substeps*min(nx,ny)+2");
     if (!nseg || !nnz) return fail(c, PCT_EINVAL, "pct_debug_rows: nseg and nnz are required");
     const void* outs[6] = {nseg, nnz, seg_idx, seg_len, row_len, nodes};
     for (int i = 0; i < 6; ++i)

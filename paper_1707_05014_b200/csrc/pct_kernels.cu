@@ -114,7 +114,7 @@ __global__ void __launch_bounds__(kThreads, kCtasPerSm) k_drop_block(const DropA
     extern __shared__ __align__(16) unsigned char smem_raw[];
     const Geom g = a.g;
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-    const SmemLayout lay = smem_layout(g.nmin);
+    const SmemLayout lay = smem_layout(g.kmax);
     float4* s_tab = reinterpret_cast<float4*>(smem_raw);
     PathState* s_state = reinterpret_cast<PathState*>(smem_raw + lay.state_off) + warp * kBatch;
     float2* row = reinterpret_cast<float2*>(smem_raw + lay.row_off) + warp * lay.row_slots;
@@ -124,7 +124,7 @@ __global__ void __launch_bounds__(kThreads, kCtasPerSm) k_drop_block(const DropA
     // else -- the block index in ctrl, the image -- is read after the wait below, i.e. after that grid has completed
     // and its writes are visible.
     asm volatile("griddepcontrol.launch_dependents;" ::: "memory");  // the update kernel may take the slots this grid's CTAs leave
-    stage_table(s_tab, a.tab, g.nmin);
+    stage_table(s_tab, a.tab, g.kmax);
     asm volatile("griddepcontrol.wait;" ::: "memory");
     if (threadIdx.x == 0) {
         long long first = a.first, count = a.count;
@@ -235,7 +235,7 @@ cudaError_t launch_drop_block(const DropArgs& a, int grid, cudaStream_t stream) 
     const long long cnt = a.first < 0 ? a.block_size : a.count;
     const long long need = (cnt + kWarpsPerCta - 1) / kWarpsPerCta;
     if (need < grid) grid = need < 1 ? 1 : (int)need;
-    const size_t smem = drop_smem_bytes(a.g.nmin);
+    const size_t smem = drop_smem_bytes(a.g.kmax);
     cudaError_t e = a.g.path_model == 1 ? launch_pdl(k_drop_block<true>, dim3(grid), dim3(kThreads), smem, stream, a)
                                         : launch_pdl(k_drop_block<false>, dim3(grid), dim3(kThreads), smem, stream, a);
     return e != cudaSuccess ? e : cudaGetLastError();
@@ -408,11 +408,11 @@ __global__ void __launch_bounds__(kThreads) k_rows(const RowsArgs a) {
     extern __shared__ __align__(16) unsigned char smem_raw[];
     const Geom g = a.g;
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-    const SmemLayout lay = smem_layout(g.nmin);
+    const SmemLayout lay = smem_layout(g.kmax);
     float4* s_tab = reinterpret_cast<float4*>(smem_raw);
     PathState* s_state = reinterpret_cast<PathState*>(smem_raw + lay.state_off) + warp * kBatch;
     float2* row = reinterpret_cast<float2*>(smem_raw + lay.row_off) + warp * lay.row_slots;
-    stage_table(s_tab, a.tab, g.nmin);
+    stage_table(s_tab, a.tab, g.kmax);
     for (long long r = (long long)blockIdx.x * kWarpsPerCta + warp; r < a.count; r += (long long)gridDim.x * kWarpsPerCta) {
         if (lane == 0) {
             const Hist hh = load_history(a.H, a.first + r);
@@ -468,8 +468,8 @@ __global__ void __launch_bounds__(kThreads) k_rows(const RowsArgs a) {
 }
 
 cudaError_t launch_rows(const RowsArgs& a, cudaStream_t stream) {
-    if (((a.g.nmin + 32) >> 5) > 64) return cudaErrorInvalidValue;
-    const size_t smem = drop_smem_bytes(a.g.nmin);
+    if (((a.g.kmax + 32) >> 5) > 64) return cudaErrorInvalidValue;
+    const size_t smem = drop_smem_bytes(a.g.kmax);
     long long blocks = (a.count + kWarpsPerCta - 1) / kWarpsPerCta;
     const long long cap = (long long)sm_count() * 8;
     if (blocks > cap) blocks = cap;

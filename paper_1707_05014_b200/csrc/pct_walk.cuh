@@ -213,7 +213,7 @@ __device__ __forceinline__ void walk_history(const Geom& g, const PathState& S, 
     const PathState st = S;  // shared memory -> registers, once per history
     const int K = st.K;
     const int C = (K + 32) >> 5;  // ceil((K + 1) / 32) segments per lane
-    const int tab_n = tab_slots(g.nmin);
+    const int tab_n = tab_slots(g.kmax);
     const int pad_mask = (C & 1) ? 0 : -1;  // odd C: the plain copy of the table, even C: the padded one
     const float4* s_tabA = s_tab + ((C & 1) ? 2 * tab_n : 0);
     const float4* s_tabB = s_tabA + tab_n;

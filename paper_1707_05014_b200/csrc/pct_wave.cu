@@ -432,16 +432,16 @@ __global__ void __launch_bounds__(kThreads, kCtasPerSm) k_wave(const __grid_cons
     const Geom g = a.g;
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     const unsigned warp_id = blockIdx.x * kWarpsPerCta + warp;
-    const SmemLayout lay = smem_layout(g.nmin);
+    const SmemLayout lay = smem_layout(g.kmax);
     float4* s_tab = reinterpret_cast<float4*>(smem_raw);
     PathState* s_state = reinterpret_cast<PathState*>(smem_raw + lay.state_off) + warp * kBatch;
     float2* row = reinterpret_cast<float2*>(smem_raw + lay.row_off) + warp * lay.row_slots;
-    stage_table(s_tab, a.tab, g.nmin);
+    stage_table(s_tab, a.tab, g.kmax);
     WaveCtrl* ctrl = a.ctrl;
     const bool planned = a.plan != nullptr;
     if (warp >= kWalkers) {  // updater warps (no CTA-wide barrier follows)
         if (planned)
-            updater_loop(a, lane, warp_id, reinterpret_cast<float4*>(smem_raw + wave_stage_off(g.nmin)) + (warp - kWalkers) * (kStageBytes / 16));
+            updater_loop(a, lane, warp_id, reinterpret_cast<float4*>(smem_raw + wave_stage_off(g.kmax)) + (warp - kWalkers) * (kStageBytes / 16));
         return;
     }
     const long long B = planned ? a.block_size : a.count;
@@ -612,7 +612,7 @@ cudaError_t launch_wave(const WaveArgs& a, int grid, cudaStream_t stream) {
     const long long items = a.plan ? (a.q1 - a.q0) * ipb : ipb;
     const long long need = (items + kWalkers - 1) / kWalkers;
     if (need < grid) grid = need < 1 ? 1 : (int)need;
-    const size_t smem = wave_smem_bytes(a.g.nmin);
+    const size_t smem = wave_smem_bytes(a.g.kmax);
     if (a.g.path_model == 1)
         k_wave<true><<<grid, kThreads, smem, stream>>>(a);
     else

@@ -63,6 +63,10 @@ def parse_args():
     ap.add_argument("--e2e-steps", type=int, default=2)
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu", action="store_true")
+    ap.add_argument("--carp", action="store_true",
+                    help="CARP across the ranks (the paper's own multi-processor scheme, PAPER.md:52-56): one string per rank, one "
+                         "all-reduce of the image per iteration; a step = one CARP iteration.  Under torchrun with --gpus N; at N = 1 "
+                         "it is one string = the DROP sweep.  A side measurement: `scaling` is strong (the N strings split one set)")
     ap.add_argument("--no-peaks", action="store_true", help="skip the L2 / fp32 micro-benchmarks behind roofline.l2")
     ap.add_argument("--peaks", action="store_true", help="only run the micro-benchmarks (pct_measure_peaks) and print them")
     ap.add_argument("--time-ordered", action="store_true",
@@ -479,6 +483,68 @@ def run_carp(args):
                                  "step": "one CARP iteration: every string one DROP sweep over its histories, then the mean"}}))
 
 
+def run_carp_ranks(args):
+    """CARP with one string per rank (replicas.carp_distributed_pct): every rank sweeps its own string of the one seeded
+    history set from the common image, then the all-reduce (sum, / world) of the image, in place on the library's array."""
+    import torch
+    import torch.distributed as dist
+
+    import paper_1707_05014_b200 as pct
+    import synth
+    import synth.cuda_gen as cuda_gen
+    from paper_1707_05014_b200 import replicas
+
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    assert torch.cuda.is_available(), "bench.py needs a CUDA device: the path has no CPU fallback"
+    torch.cuda.set_device(local)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+    cfg = synth.config(args.config)
+    n = cfg.n if args.histories is None else int(args.histories)
+    lo, hi = replicas.string_range(rank, world, n)  # R27: contiguous balanced strings of the caller's order
+    D = synth.to_pct_names(cuda_gen.generate_cuda(cfg, hi - lo, first=lo))
+    stream = torch.cuda.Stream()
+    with torch.cuda.stream(stream):
+        ctx = pct.pct_create(cfg.nx, cfg.ny, cfg.nz, cfg.h, cfg.u_in, cfg.u_out, stream.cuda_stream)
+        try:
+            pct.pct_set_histories(ctx, hi - lo, D)
+            _, n_slots = pct.pct_image_storage(ctx)
+            replicas.carp_distributed_pct(pct, ctx, cfg.n_voxels, cfg.lam, cfg.block_size, args.warmup, world, stream.cuda_stream)
+            pct.pct_synchronize(ctx)
+            replicas.barrier(world)
+            torch.cuda.synchronize()
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            with ClockSampler(local) as clk:
+                e0.record()
+                replicas.carp_distributed_pct(pct, ctx, cfg.n_voxels, cfg.lam, cfg.block_size, args.steps, world, stream.cuda_stream)
+                e1.record()
+                torch.cuda.synchronize()
+                replicas.barrier(world)
+            ms = replicas.max_over_ranks(e0.elapsed_time(e1), world, "cuda")
+            img = torch.empty(cfg.n_voxels, dtype=torch.float32, device="cuda")
+            pct.pct_get_image(ctx, img, cfg.n_voxels)
+            finite = bool(torch.isfinite(img).all().item())
+        finally:
+            pct.pct_destroy(ctx)
+    if world > 1:
+        dist.destroy_process_group()
+    if rank != 0:
+        return
+    n_blocks = ((hi - lo) + cfg.block_size - 1) // cfg.block_size
+    print(json.dumps({
+        "metric": METRIC, "value": n * args.steps / (ms * 1e-3), "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
+        "ms_per_step": ms / args.steps, "higher_is_better": True, "scaling": "strong", "vs_baseline": None, "dtype": "f32",
+        "data": "synthetic", "clocks": clk.summary(), "gpu_launches": 2 * n_blocks * args.steps, "image_finite": finite,
+        "comm": {"collective": "all-reduce (sum) of the image, in place on the library's array" if world > 1 else "none (one string)",
+                 "bytes_per_rank_per_step": 4 * n_slots if world > 1 else 0},
+        "config": {"workload": cfg.workload, "algorithm": "CARP, one string per rank (PAPER.md:52-56; DESIGN.md R27-R29)",
+                   "strings": world, "histories": n, "histories_per_rank": hi - lo, "block_size": cfg.block_size, "lambda": cfg.lam,
+                   "step": "one CARP iteration: every rank one DROP sweep over its string from the common image, then the average",
+                   "note": "side measurement, not the driver's contract; unmeasured on N > 1 in this repository's runs (one GPU per run)"}}))
+
+
 def run_peaks(args):
     """Only the micro-benchmarks behind roofline.l2 (pct_measure_peaks), on an L2-resident footprint and on the
     footprint of image + accumulator of the config."""
@@ -500,6 +566,8 @@ def main():
     args = parse_args()
     if args.peaks:
         run_peaks(args)
+    elif args.carp and args.impl != "reference":
+        run_carp_ranks(args)
     elif args.carp_strings > 0 and args.impl != "reference":
         run_carp(args)
     elif args.impl == "reference":

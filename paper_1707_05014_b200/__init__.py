@@ -18,6 +18,7 @@ from .binding import (  # noqa: F401
     pct_get_image,
     pct_get_stats,
     pct_get_tvs_state,
+    pct_image_storage,
     pct_iterate,
     pct_iterate_carp,
     pct_measure_peaks,

@@ -1001,6 +1001,13 @@ extern "C" int pct_set_image(pct_ctx* c, const float* src, int64_t n_voxels) {
     return PCT_OK;
 }
 
+extern "C" int pct_image_storage(pct_ctx* c, float** image, int64_t* n_slots) {
+    if (!c || !image || !n_slots) return PCT_EINVAL;
+    *image = c->x;
+    *n_slots = c->n_slots;
+    return PCT_OK;
+}
+
 extern "C" int pct_get_stats(pct_ctx* c, int64_t out[4]) {
     if (!c || !out) return PCT_EINVAL;
     DeviceGuard guard(c->device);

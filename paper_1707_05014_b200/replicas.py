@@ -67,13 +67,23 @@ def carp_distributed(sweep, get_image, set_image, n_iter, world):
         set_image(x)
 
 
-def carp_distributed_pct(pct, ctx, n_voxels, lam, block_size, n_iter, world):
-    """carp_distributed on a libpct context holding this rank's string (pct = the binding module)."""
-    buf = torch.empty(int(n_voxels), dtype=torch.float32, device="cuda")
+class _DeviceArray:
+    """A borrowed device array as something torch.as_tensor understands (no copy)."""
 
-    def get_image():
-        pct.pct_get_image(ctx, buf, n_voxels)
-        return buf
+    def __init__(self, address, n):
+        self.__cuda_array_interface__ = {"shape": (int(n),), "typestr": "<f4", "data": (int(address), False), "version": 3}
 
-    carp_distributed(lambda: pct.pct_iterate(ctx, lam, block_size, 1), get_image,
-                     lambda t: pct.pct_set_image(ctx, t, n_voxels), n_iter, world)
+
+def carp_distributed_pct(pct, ctx, n_voxels, lam, block_size, n_iter, world, ctx_stream=None):
+    """carp_distributed on a libpct context holding this rank's string (pct = the binding module).
+
+    The average is taken IN PLACE on the library's own image array (pct_image_storage: the storage order is the same
+    on every rank of the same grid, and a sum does not care about order): no copy, no host synchronisation.  All of it
+    is ordered on the context's stream: ctx_stream is the cudaStream_t handle given to pct_create (None: the context was
+    created on torch's current stream), and the collective and the division run under that stream, so the sweep, the
+    all-reduce and the next sweep follow one another on the device."""
+    address, n_slots = pct.pct_image_storage(ctx)
+    x = torch.as_tensor(_DeviceArray(address, n_slots), device="cuda")
+    stream = torch.cuda.current_stream() if ctx_stream is None else torch.cuda.ExternalStream(int(ctx_stream))
+    with torch.cuda.stream(stream):
+        carp_distributed(lambda: pct.pct_iterate(ctx, lam, block_size, 1), lambda: x, lambda t: None, n_iter, world)

@@ -571,3 +571,46 @@ def test_error_reporting(pct, torch_cuda):
         pct.pct_synchronize(ctx)
     finally:
         pct.pct_destroy(ctx)
+
+
+def test_carp_across_two_contexts_averaged_in_place_is_carp_with_two_strings(oracle_mod, pct, torch_cuda):
+    """The multi-GPU form of CARP (replicas.carp_distributed_pct: one string per rank, the average taken in place on the
+    library's own image array) with the two ranks played by two contexts of ONE process, one after the other (their
+    kernels never wait on one another): the all-reduce is written out as the sum of the two storage arrays / 2.
+    Must equal pct_iterate_carp(P = 2) on one context and the oracle's CARP with two strings."""
+    from paper_1707_05014_b200 import replicas
+
+    torch = torch_cuda
+    cfg = synth.config(0)
+    n, B, lam, iters = 30_011, 700, 0.5, 3
+    H = synth.generate_numpy(cfg, n)
+    D = to_device(H)
+    M = cfg.n_voxels
+    tables = ("proj_cos", "proj_sin")
+    ctxs, xs = [], []
+    try:
+        for r in range(2):
+            lo, hi = replicas.string_range(r, 2, n)
+            Dr = {k: (v if k in tables else v[lo:hi]) for k, v in D.items()}
+            c = _ctx(pct, torch, cfg)
+            ctxs.append((c, Dr))
+            pct.pct_set_histories(c, hi - lo, Dr)
+            addr, n_slots = pct.pct_image_storage(c)
+            xs.append(torch.as_tensor(replicas._DeviceArray(addr, n_slots), device="cuda"))
+        assert xs[0].numel() >= M and xs[0].numel() == xs[1].numel()
+        for _ in range(iters):
+            for c, _d in ctxs:
+                pct.pct_iterate(c, lam, B, 1)
+            mean = (xs[0] + xs[1]) / 2  # what all_reduce(sum) followed by /= world leaves on every rank
+            xs[0].copy_(mean)
+            xs[1].copy_(mean)
+        out = torch.zeros(M, dtype=torch.float32, device="cuda")
+        pct.pct_get_image(ctxs[1][0], out, M)
+        got = out.cpu().numpy().astype(np.float64)
+    finally:
+        for c, _d in ctxs:
+            pct.pct_destroy(c)
+    geom = oracle_geom(oracle_mod, cfg)
+    x_ref = oracle_mod.carp_iterate(geom, oracle_mod.Histories(H), lam, B, iters, 2, np.zeros(M))
+    assert np.linalg.norm(got - x_ref) <= REL_L2_PER_ITER * np.linalg.norm(x_ref)
+    assert np.abs(got - x_ref).max() <= ABS_FINAL

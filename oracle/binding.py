@@ -21,6 +21,10 @@ def _flags():
                 flags.append("-mfma")  # fmaf() -> one vfmadd; without it glibc's exact fmaf is called
     except OSError:
         pass
+    # ORACLE_SANITIZE=1: AddressSanitizer + UndefinedBehaviorSanitizer build of the checker (run the CPU tests with
+    # LD_PRELOAD=$(gcc -print-file-name=libasan.so) ASAN_OPTIONS=detect_leaks=0; profiles/r2_sanitizers.md)
+    if os.environ.get("ORACLE_SANITIZE"):
+        flags += ["-g", "-fsanitize=address,undefined", "-fno-omit-frame-pointer"]
     return flags
 
 

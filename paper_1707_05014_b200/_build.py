@@ -40,6 +40,8 @@ def _tag():
 
 def build(force=False, verbose=False):
     """Compile csrc/*.cu -> paper_1707_05014_b200/libpct.so (rebuilt when sources or flags change)."""
+    if os.environ.get("PCT_LIB"):  # a prebuilt library (a checking or profiling build of the same sources)
+        return os.environ["PCT_LIB"]
     tag = _tag()
     if not force and os.path.exists(LIB) and os.path.exists(_STAMP):
         with open(_STAMP) as f:

@@ -869,8 +869,11 @@ extern "C" int pct_iterate_carp(pct_ctx* c, float lambda, int64_t block_size, in
             CUDA_TRY(c, cudaStreamWaitEvent(c->stream, c->carp_done[p], 0));
         }
         CUDA_TRY(c, launch_mean(c->x, c->carp_x, P, M, stride, c->stream));
-        if (c->engine == 1)  // pct_get_stats: the counters of the strings' sweeps, added up
-            CUDA_TRY(c, launch_sum_stats(c->wctrl, c->carp_wctrl, P, c->stream));
+        // pct_get_stats: the counters of the strings' sweeps, added up
+        if (c->engine == 1)
+            CUDA_TRY(c, launch_sum_stats(c->wctrl->last, c->carp_wctrl[0].last, sizeof(WaveCtrl), P, c->stream));
+        else
+            CUDA_TRY(c, launch_sum_stats(c->ctrl->last, c->carp_ctrl[0].last, sizeof(Ctrl), P, c->stream));
     }
     return PCT_OK;
 }
@@ -1018,6 +1021,7 @@ extern "C" int pct_get_stats(pct_ctx* c, int64_t out[4]) {
     for (int i = 0; i < 3; ++i) out[i] = (int64_t)last[i];
     out[3] = c->n;
     wave_prof_dump("pct_get_stats");
+    bounds_dump("pct_get_stats");
     return check_wave_error(c);
 }
 

@@ -52,6 +52,7 @@ struct RowsArgs {
 
 // launchers (pct_kernels.cu); all asynchronous on `stream`, return the launch error
 size_t drop_smem_bytes(int nmin);
+void bounds_dump(const char* tag);  // (a no-op unless built with -DPCT_CHECK_BOUNDS)
 cudaError_t drop_configure(int nmin, int* grid_out);
 cudaError_t launch_drop_block(const DropArgs& a, int grid, cudaStream_t stream);
 cudaError_t launch_update(float* x, float2* acc, long long n_voxels, float lambda, Ctrl* ctrl,
@@ -120,7 +121,7 @@ int wave_walkers_per_cta();
 size_t wave_smem_need(int nmin);
 cudaError_t wave_configure(int nmin, int* grid_out);
 void wave_prof_dump(const char* tag);  // (a no-op unless built with -DPCT_WAVE_PROF)
-cudaError_t launch_sum_stats(WaveCtrl* dst, const WaveCtrl* strings, int n_strings, cudaStream_t stream);
+cudaError_t launch_sum_stats(unsigned long long* dst, const unsigned long long* src, size_t pitch, int n_strings, cudaStream_t stream);
 cudaError_t launch_wave(const WaveArgs& a, int grid, cudaStream_t stream);
 cudaError_t launch_plan_blocks(const HistPtrs& H, const Geom& g, long long n, long long block_size, long long first_block,
                                long long n_blocks, const WaveShape& shp, uint32_t* plan, int* need, cudaStream_t stream);

@@ -13,13 +13,24 @@
 //                 path is computed once per sweep and never touches global memory.
 //   k_update      x_j += lambda * Delta_j / max(1, c_j); accumulator zeroed; DROP block index advanced.
 //   k_rows        inspection: the same walk, rows written out instead of consumed.
+#include <stdio.h>
 #include <stdlib.h>
+#include <string.h>
 
 #include "pct_walk.cuh"
 
 namespace pct {
 
 size_t drop_smem_bytes(int nmin) { return (size_t)smem_layout(nmin).total; }
+
+// (checking build only) print and clear the violation counters of the block engine's kernels
+void bounds_dump(const char* tag) {
+#ifdef PCT_CHECK_BOUNDS
+    bounds_dump_tu(tag);
+#else
+    (void)tag;
+#endif
+}
 
 static int sm_count() {
     int dev = 0, sms = 0;
@@ -153,6 +164,7 @@ __global__ void __launch_bounds__(kThreads, kCtasPerSm) k_drop_block(const DropA
         if (lane < cnt) {
             long long r = rel0 + lane * stride;  // position in the processing order of the block
             if (q.interleave) r = (long long)__ldg(a.order + q.first + r);  // ordered block (k_order_blocks)
+            PCT_BOUND(3, q.first + r >= 0 && q.first + r < a.n);
             const Hist hh = load_history(a.H, q.first + r);
             setup_history(g, hh, s_state[lane]);
         }
@@ -601,17 +613,19 @@ cudaError_t launch_mean(float* x, const float* xs, int n_strings, long long n, l
     return cudaGetLastError();
 }
 
-// pct_get_stats after CARP: the counters of the strings' last sweeps, added up into the context's.
-__global__ void k_sum_stats(WaveCtrl* dst, const WaveCtrl* strings, int n_strings) {
+// pct_get_stats after CARP: the counters of the strings' last sweeps, added up into the context's.  src = the `last`
+// array of string 0, the strings' control blocks `pitch` bytes apart.
+__global__ void k_sum_stats(unsigned long long* dst, const unsigned long long* src, size_t pitch, int n_strings) {
     if (threadIdx.x < 4) {
         unsigned long long s = 0;
-        for (int p = 0; p < n_strings; ++p) s += strings[p].last[threadIdx.x];
-        dst->last[threadIdx.x] = s;
+        for (int p = 0; p < n_strings; ++p)
+            s += reinterpret_cast<const unsigned long long*>(reinterpret_cast<const char*>(src) + (size_t)p * pitch)[threadIdx.x];
+        dst[threadIdx.x] = s;
     }
 }
 
-cudaError_t launch_sum_stats(WaveCtrl* dst, const WaveCtrl* strings, int n_strings, cudaStream_t stream) {
-    k_sum_stats<<<1, 32, 0, stream>>>(dst, strings, n_strings);
+cudaError_t launch_sum_stats(unsigned long long* dst, const unsigned long long* src, size_t pitch, int n_strings, cudaStream_t stream) {
+    k_sum_stats<<<1, 32, 0, stream>>>(dst, src, pitch, n_strings);
     return cudaGetLastError();
 }
 

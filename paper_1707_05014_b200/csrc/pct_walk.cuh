@@ -3,9 +3,30 @@
 // buffer, the lane-chunked walk of one history by one warp (rule steps 3-4) and the segment-major
 // gather (a_i.x) and scatter ((Delta_j, c_j) += ...) passes (R12).
 #pragma once
+#include <stdio.h>
+
 #include "pct_internal.h"
 
 namespace pct {
+
+// Build with -DPCT_CHECK_BOUNDS for a checking build (compute-sanitizer is closed on this pool: profiles/r2_sanitizers.md):
+// every storage slot the walk produces, every row-buffer and table index it forms and every history index it loads
+// is tested against its array, violations are counted per kind and reported by bounds_dump().
+#ifdef PCT_CHECK_BOUNDS
+static __device__ unsigned long long g_pct_bounds[8];  // (one copy per translation unit)
+#define PCT_BOUND(kind, ok) do { if (!(ok)) atomicAdd(&g_pct_bounds[kind], 1ULL); else if ((kind) == 0) atomicAdd(&g_pct_bounds[4], 1ULL); } while (0)
+// print and clear this translation unit's counters
+static inline void bounds_dump_tu(const char* tag) {
+    unsigned long long h[8] = {0};
+    cudaMemcpyFromSymbol(h, g_pct_bounds, sizeof(h));
+    fprintf(stderr, "[bounds %s] segment pairs checked %llu; violations: voxel slot %llu, row buffer %llu, table %llu, history index %llu\n", tag,
+            h[4], h[0], h[1], h[2], h[3]);
+    for (int i = 0; i < 8; ++i) h[i] = 0;
+    cudaMemcpyToSymbol(g_pct_bounds, h, sizeof(h));
+}
+#else
+#define PCT_BOUND(kind, ok)
+#endif
 
 #ifndef PCT_WARPS_PER_CTA
 #define PCT_WARPS_PER_CTA 10
@@ -192,8 +213,11 @@ __device__ __forceinline__ void take_two(const Geom& g, const Node2& a, const No
                                          unsigned row_sa, const EmitPtrs& em) {
     f2 len, gx, gy, gz;
     segment2(g, a, b, len, gx, gy, gz);
-    if (first) take_segment<EMIT>(voxel_of(g, lo_of(gx), lo_of(gy), lo_of(gz)), lo_of(len), lo3(a), seg, K, m, row_sa, em);
-    take_segment<EMIT>(voxel_of(g, hi_of(gx), hi_of(gy), hi_of(gz)), hi_of(len), hi3(a), seg + 1, K, m, row_sa, em);
+    const int lin_lo = voxel_of(g, lo_of(gx), lo_of(gy), lo_of(gz)), lin_hi = voxel_of(g, hi_of(gx), hi_of(gy), hi_of(gz));
+    PCT_BOUND(0, lin_lo >= -1 && lin_lo < g.slice_p * g.nz && lin_hi >= -1 && lin_hi < g.slice_p * g.nz);  // a slot of image / accumulator
+    PCT_BOUND(1, (first ? seg : seg + 1) >= 0 && row_slot(seg + 1) < row_slots((g.kmax + 32) >> 5));        // the warp's row buffer
+    if (first) take_segment<EMIT>(lin_lo, lo_of(len), lo3(a), seg, K, m, row_sa, em);
+    take_segment<EMIT>(lin_hi, hi_of(len), hi3(a), seg + 1, K, m, row_sa, em);
 }
 
 // Walk of one history by one warp (steps 3-4 of the rule): fills the warp's row buffer, returns the
@@ -218,6 +242,7 @@ __device__ __forceinline__ void walk_history(const Geom& g, const PathState& S, 
     const float4* s_tabA = s_tab + ((C & 1) ? 2 * tab_n : 0);
     const float4* s_tabB = s_tabA + tab_n;
     const int k0 = lane * C;
+    PCT_BOUND(2, tab_slot(k0 + C - 1) < tab_n && C <= ((g.kmax + 32) >> 5));  // the staged table (its last entry read by this lane)
     const float3 exitP = to_object(st, st.t2, st.u2, st.v2);  // node K+1: the hull exit point, assigned (R9)
     const Node2 Z = node_pair<SPLINE>(st, s_tabA, s_tabB, pad_mask, k0 + C - 1, K, exitP);
     const float3 last = hi3(Z);

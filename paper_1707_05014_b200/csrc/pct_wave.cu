@@ -471,6 +471,7 @@ __global__ void __launch_bounds__(kThreads, kCtasPerSm) k_wave(const __grid_cons
                 r = (long long)(code & 0xffffffu);
                 plan_decode(code, a.n_slabs, my_sa, my_sb);
             }
+            PCT_BOUND(3, first + r >= 0 && first + r < a.n + (planned ? 0 : a.first));
             const Hist hh = load_history(a.H, first + r);
             setup_history(g, hh, s_state[lane]);
         }
@@ -552,6 +553,9 @@ __global__ void __launch_bounds__(kThreads, kCtasPerSm) k_wave(const __grid_cons
 }
 
 void wave_prof_dump(const char* tag) {
+#ifdef PCT_CHECK_BOUNDS
+    bounds_dump_tu("wavefront engine");
+#endif
 #ifdef PCT_WAVE_PROF
     unsigned long long h[16] = {0};
     cudaMemcpyFromSymbol(h, g_wave_prof, sizeof(h));

@@ -262,6 +262,11 @@ def _carp_parity(oracle, pct, torch, cfg, H, lam, block, n_iter, n_strings, x0=N
             rel = np.linalg.norm(x - x_ref) / np.linalg.norm(x_ref)
             assert rel <= REL_L2_PER_ITER, "iteration %d: rel L2 %.3g" % (it, rel)
         assert np.abs(x - x_ref).max() <= ABS_FINAL
+        # the counters of the last iteration: the strings' sweeps added up = one sweep over all histories (rows and
+        # non-zeros are properties of the paths, not of the image)
+        _, st = oracle.drop_iterate(geom, hs, lam, block, 1, np.zeros(M))
+        gs = pct.pct_get_stats(ctx)
+        assert (gs["rows"], gs["nnz"]) == st
     finally:
         pct.pct_destroy(ctx)
     return x, x_ref

@@ -16,6 +16,7 @@ from .binding import (  # noqa: F401
     drop_iterate,
     get_path_model,
     get_substeps,
+    get_walk_mode,
     lib,
     mlp_chi2_f64,
     mlp_matrix_f64,
@@ -26,6 +27,7 @@ from .binding import (  # noqa: F401
     scatter_f,
     set_path_model,
     set_substeps,
+    set_walk_mode,
     sigma1_table,
     sigma_f64,
     xyz_to_beam_f32,

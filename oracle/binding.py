@@ -213,26 +213,27 @@ def row_f32(geom, hist, table=None):
     if table is None:
         table = sigma1_table(geom.h / get_substeps(), get_substeps() * geom.nmin)
     ms = get_substeps() * geom.nmin + 2
-    row_idx = np.zeros(ms, dtype=np.int32)
-    row_len = np.zeros(ms, dtype=np.float32)
-    seg_idx = np.zeros(ms, dtype=np.int32)
-    seg_len = np.zeros(ms, dtype=np.float32)
+    cap = ms if get_walk_mode() == 0 else 8 * ms
+    row_idx = np.zeros(cap, dtype=np.int32)
+    row_len = np.zeros(cap, dtype=np.float32)
+    seg_idx = np.zeros(cap, dtype=np.int32)
+    seg_len = np.zeros(cap, dtype=np.float32)
     nodes = np.zeros((ms + 1, 3), dtype=np.float32)
     coefs = np.zeros((ms + 1, 2), dtype=np.float32)
     nseg = C.c_int(0)
     ip = C.POINTER(C.c_int32)
     g, h = geom.c(), hist
-    rc = lib().orc_row_f32(C.byref(g), C.byref(h), *[a.ctypes.data_as(_FP) for a in table], ms,
+    rc = lib().orc_row_f32(C.byref(g), C.byref(h), *[a.ctypes.data_as(_FP) for a in table], cap,
                            row_idx.ctypes.data_as(ip), row_len.ctypes.data_as(_FP),
                            seg_idx.ctypes.data_as(ip), seg_len.ctypes.data_as(_FP),
                            nodes.ctypes.data_as(_FP), coefs.ctypes.data_as(_FP), C.byref(nseg))
     if rc < 0:
         raise RuntimeError("segment buffer too small: need %d" % -rc)
-    ns = nseg.value
+    ns = nseg.value  # items of the row before merging: segments (midpoint rule) or pieces (exact traversal)
+    nn = int(lib().orc_node_count(C.byref(g), C.byref(h))) if ns else 0
     return dict(nnz=rc, nseg=ns, row_idx=row_idx[:rc].copy(), row_len=row_len[:rc].copy(),
                 seg_idx=seg_idx[:ns].copy(), seg_len=seg_len[:ns].copy(),
-                nodes=nodes[:ns + 1].copy() if ns else nodes[:0].copy(),
-                coefs=coefs[:ns + 1].copy() if ns else coefs[:0].copy())
+                nodes=nodes[:nn].copy(), coefs=coefs[:nn].copy())
 
 
 def block_accumulate(geom, hists, first, count, x, nthreads=0):
@@ -323,3 +324,12 @@ def set_substeps(n):
 
 def get_substeps():
     return int(lib().orc_get_substeps())
+
+
+def set_walk_mode(mode):
+    """0: midpoint rule (R10, default); 1: exact traversal of the polyline (R34).  Process-wide."""
+    lib().orc_set_walk_mode(int(mode))
+
+
+def get_walk_mode():
+    return int(lib().orc_get_walk_mode())

@@ -503,6 +503,77 @@ static void r32_node(const orc_geom *g, const orc_hist *hh, const r32_state *st,
  *   coefs            (optional) (K+2) x 2 fp32 MLP coefficients c0, c2 (0 for the end nodes)
  * Returns nnz of the merged row (0 for a skipped history), or -needed if max_seg < K+1.
  * *nseg_out = K+1 (0 if skipped). */
+/* ==========================================================================================
+ * Walk mode (R34).  0: the midpoint rule of R10 (a segment's length goes to the
+ * voxel of its midpoint), the graded path.  1: EXACT traversal of the polyline: every segment A -> B is cut at
+ * the voxel faces it crosses and every piece goes to the voxel it lies in, so that the row is the list of the
+ * polyline's chord lengths.  fp32, this operation order (it decides voxel indices):
+ *     gA = fma(A, 1/h, n/2), gB likewise, d = gB - gA                       (grid coordinates, per axis)
+ *     for axis x, y, z: if floor(gA) != floor(gB): for every integer p, min + 1 <= p <= max of the two floors,
+ *         ascending: t = (p - gA) / d, clamped to [0, 1]                    (at most ORC_MAX_CUTS cuts in all)
+ *     cuts sorted ascending; consecutive cuts t0 < t1 (0 and 1 included) give a piece of length (t1 - t0) * len
+ *     in the voxel floor(fma(0.5 (t0 + t1), d, gA)); pieces of zero length are dropped
+ * The row merges consecutive equal voxels as before (a piece outside the grid breaks a run).
+ * ======================================================================================== */
+#define ORC_MAX_CUTS 24
+static int g_walk_mode = 0;
+void orc_set_walk_mode(int m) { g_walk_mode = m == 1 ? 1 : 0; }
+int orc_get_walk_mode(void) { return g_walk_mode; }
+int orc_row_capacity(const orc_geom *g) { return g_walk_mode == 1 ? 8 * (orc_kmax(g) + 2) : orc_kmax(g) + 2; }
+
+static int32_t r32_voxel(const orc_geom *g, float gx, float gy, float gz) {
+    const float fx = floorf(gx), fy = floorf(gy), fz = floorf(gz);
+    if (fx >= 0.0f && fx < (float)g->nx && fy >= 0.0f && fy < (float)g->ny && fz >= 0.0f && fz < (float)g->nz)
+        return (int32_t)fx + g->nx * ((int32_t)fy + g->ny * (int32_t)fz);
+    return -1;
+}
+
+static int r32_pieces(const orc_geom *g, const float A[3], const float B[3], float len, int32_t *vox, float *plen) {
+    const float inv_h = 1.0f / g->h;
+    const float half[3] = {0.5f * (float)g->nx, 0.5f * (float)g->ny, 0.5f * (float)g->nz};
+    float ga[3], d[3], ts[ORC_MAX_CUTS];
+    int nt = 0;
+    for (int c = 0; c < 3; ++c) {
+        ga[c] = fmaf(A[c], inv_h, half[c]);
+        const float gb = fmaf(B[c], inv_h, half[c]);
+        d[c] = gb - ga[c];
+        const float fa = floorf(ga[c]), fb = floorf(gb);
+        if (fa != fb) {
+            const float lo = fa < fb ? fa : fb, hi = fa < fb ? fb : fa;
+            for (float p = lo + 1.0f; p <= hi && nt < ORC_MAX_CUTS; p += 1.0f) {
+                float t = (p - ga[c]) / d[c];
+                t = t < 0.0f ? 0.0f : (t > 1.0f ? 1.0f : t);
+                ts[nt++] = t;
+            }
+        }
+    }
+    for (int i = 1; i < nt; ++i) { /* insertion sort, ascending */
+        const float v = ts[i];
+        int j = i - 1;
+        while (j >= 0 && ts[j] > v) { ts[j + 1] = ts[j]; --j; }
+        ts[j + 1] = v;
+    }
+    int np = 0;
+    float t0 = 0.0f;
+    for (int j = 0; j <= nt; ++j) {
+        const float t1 = j < nt ? ts[j] : 1.0f;
+        if (t1 > t0) {
+            const float tm = 0.5f * (t0 + t1);
+            vox[np] = r32_voxel(g, fmaf(tm, d[0], ga[0]), fmaf(tm, d[1], ga[1]), fmaf(tm, d[2], ga[2]));
+            plen[np] = (t1 - t0) * len;
+            ++np;
+            t0 = t1;
+        }
+    }
+    return np;
+}
+
+/* number of nodes K + 2 of the fp32 path of a history (0: skipped) */
+int orc_node_count(const orc_geom *g, const orc_hist *hh) {
+    r32_state st;
+    return r32_setup(g, hh, &st) ? st.K + 2 : 0;
+}
+
 int orc_row_f32(const orc_geom *g, const orc_hist *hh, const float *p11t, const float *p12t,
                 const float *p22t, int max_seg, int32_t *row_idx, float *row_len, int32_t *seg_idx,
                 float *seg_len, float *nodes, float *coefs, int *nseg_out) {
@@ -514,8 +585,8 @@ int orc_row_f32(const orc_geom *g, const orc_hist *hh, const float *p11t, const 
     const float inv_h = 1.0f / g->h;
     const float hx = 0.5f * (float)g->nx, hy = 0.5f * (float)g->ny, hz = 0.5f * (float)g->nz;
     float prev[3], cur[3];
-    int nnz = 0;
-    int32_t last = -1; /* index of the previous segment in k (-1: none or dropped) */
+    int nnz = 0, ns = 0; /* ns: items (segments, or pieces in the exact mode) emitted so far */
+    int32_t last = -1;   /* voxel of the previous item (-1: none or dropped) */
     r32_node(g, hh, &st, 0, p11t, p12t, p22t, prev);
     if (nodes) memcpy(nodes, prev, 12);
     if (coefs) { coefs[0] = 0.0f; coefs[1] = 0.0f; }
@@ -530,30 +601,36 @@ int orc_row_f32(const orc_geom *g, const orc_hist *hh, const float *p11t, const 
         }
         const float dx = cur[0] - prev[0], dy = cur[1] - prev[1], dz = cur[2] - prev[2];
         const float len = sqrtf(fmaf(dz, dz, fmaf(dy, dy, dx * dx)));
-        const float gx = fmaf(0.5f * (prev[0] + cur[0]), inv_h, hx);
-        const float gy = fmaf(0.5f * (prev[1] + cur[1]), inv_h, hy);
-        const float gz = fmaf(0.5f * (prev[2] + cur[2]), inv_h, hz);
-        const float fx = floorf(gx), fy = floorf(gy), fz = floorf(gz);
-        int32_t lin = -1;
-        if (fx >= 0.0f && fx < (float)g->nx && fy >= 0.0f && fy < (float)g->ny && fz >= 0.0f &&
-            fz < (float)g->nz)
-            lin = (int32_t)fx + g->nx * ((int32_t)fy + g->ny * (int32_t)fz);
-        if (seg_idx) seg_idx[k] = lin;
-        if (seg_len) seg_len[k] = len;
-        if (lin >= 0) {
-            if (lin == last) {
-                /* merged in double by the callers that need it; here in fp32 for the debug row */
-                if (row_len) row_len[nnz - 1] += len;
-            } else {
-                if (row_idx) row_idx[nnz] = lin;
-                if (row_len) row_len[nnz] = len;
-                ++nnz;
-            }
+        int32_t pv[ORC_MAX_CUTS + 1];
+        float pl[ORC_MAX_CUTS + 1];
+        int np = 1;
+        if (g_walk_mode == 1) {
+            np = r32_pieces(g, prev, cur, len, pv, pl);
+        } else {
+            pv[0] = r32_voxel(g, fmaf(0.5f * (prev[0] + cur[0]), inv_h, hx), fmaf(0.5f * (prev[1] + cur[1]), inv_h, hy),
+                              fmaf(0.5f * (prev[2] + cur[2]), inv_h, hz));
+            pl[0] = len;
         }
-        last = lin;
+        if (ns + np > max_seg) return -(ns + np);
+        for (int j = 0; j < np; ++j, ++ns) {
+            const int32_t lin = pv[j];
+            if (seg_idx) seg_idx[ns] = lin;
+            if (seg_len) seg_len[ns] = pl[j];
+            if (lin >= 0) {
+                if (lin == last) {
+                    /* merged in double by the callers that need it; here in fp32 for the debug row */
+                    if (row_len) row_len[nnz - 1] += pl[j];
+                } else {
+                    if (row_idx) row_idx[nnz] = lin;
+                    if (row_len) row_len[nnz] = pl[j];
+                    ++nnz;
+                }
+            }
+            last = lin;
+        }
         memcpy(prev, cur, 12);
     }
-    if (nseg_out) *nseg_out = K + 1;
+    if (nseg_out) *nseg_out = ns;
     return nnz;
 }
 
@@ -607,7 +684,7 @@ int orc_block_accumulate(const orc_geom *g, const orc_histories *H, int64_t firs
                          const double *x, double *delta, int32_t *cnt, int64_t *stats,
                          int nthreads) {
     const int nmin = orc_kmax(g); /* (most interior nodes a path can have) */
-    const int max_seg = nmin + 2;
+    const int max_seg = orc_row_capacity(g);
     const int64_t M = (int64_t)g->nx * g->ny * g->nz;
     float *p11t = (float *)malloc(sizeof(float) * (nmin + 1));
     float *p12t = (float *)malloc(sizeof(float) * (nmin + 1));

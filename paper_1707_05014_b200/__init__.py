@@ -9,6 +9,8 @@ from .binding import (  # noqa: F401
     FIELDS,
     PCT_PATH_MLP,
     PCT_PATH_SPLINE,
+    PCT_WALK_EXACT,
+    PCT_WALK_MIDPOINT,
     PctError,
     lib,
     pct_create,
@@ -30,6 +32,7 @@ from .binding import (  # noqa: F401
     pct_set_path_model,
     pct_set_step,
     pct_set_tvs,
+    pct_set_walk,
     pct_synchronize,
     pct_tvs_step,
     pct_version,

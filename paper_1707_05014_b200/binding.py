@@ -72,6 +72,7 @@ def lib():
         L.pct_measure_peaks.argtypes = [vp, i64, C.POINTER(C.c_double)]
         L.pct_set_tvs.argtypes = [vp, C.c_float, C.c_float, C.c_int]
         L.pct_set_step.argtypes = [vp, C.c_int]
+        L.pct_set_walk.argtypes = [vp, C.c_int]
         L.pct_image_storage.argtypes = [vp, C.POINTER(vp), C.POINTER(i64)]
         L.pct_tvs_step.argtypes = [vp]
         L.pct_get_tvs_state.argtypes = [vp, C.POINTER(C.c_double)]
@@ -81,7 +82,7 @@ def lib():
 
 EXPORTS = ("pct_create", "pct_set_histories", "pct_set_histories_host", "pct_set_histories_xyz", "pct_iterate", "pct_iterate_carp", "pct_set_path_model", "pct_get_image",
            "pct_set_image", "pct_synchronize", "pct_get_stats", "pct_destroy", "pct_last_error", "pct_version",
-           "pct_debug_rows", "pct_debug_block", "pct_profile_sweep", "pct_measure_peaks", "pct_set_tvs", "pct_tvs_step", "pct_set_step", "pct_image_storage",
+           "pct_debug_rows", "pct_debug_block", "pct_profile_sweep", "pct_measure_peaks", "pct_set_tvs", "pct_tvs_step", "pct_set_step", "pct_set_walk", "pct_image_storage",
            "pct_get_tvs_state")
 
 
@@ -234,3 +235,11 @@ def pct_image_storage(ctx):
     p, n = C.c_void_p(), C.c_int64()
     _check(ctx, lib().pct_image_storage(ctx, C.byref(p), C.byref(n)))
     return int(p.value), int(n.value)
+
+
+PCT_WALK_MIDPOINT, PCT_WALK_EXACT = 0, 1
+
+
+def pct_set_walk(ctx, mode):
+    """PCT_WALK_MIDPOINT (default) or PCT_WALK_EXACT: exact traversal of the path polyline (include/pct.h)."""
+    _check(ctx, lib().pct_set_walk(ctx, int(mode)))

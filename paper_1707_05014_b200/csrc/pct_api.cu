@@ -82,6 +82,9 @@ struct pct_ctx {
     std::vector<WavePlan> plans;   // one per string (one for DROP)
     WaveCtrl* carp_wctrl = nullptr;
     long long carp_stride = 0;     // voxels between the images / accumulators of two strings (a multiple of four)
+    // exact-traversal walk (pct_set_walk): scratch of the lanes' runs, nullptr in the default (midpoint) mode
+    float2* exact_scratch = nullptr;
+    int exact_cap = 0;
     // total-variation superiorization (pct_set_tvs): off unless tvs_beta0 > 0
     float tvs_beta0 = 0.f, tvs_gamma = 1.f;
     int tvs_levels = 0, tvs_parity = 0;
@@ -98,6 +101,7 @@ struct pct_ctx {
 
 static thread_local char g_create_err[512] = {0};
 static int tvs_step(pct_ctx* c, float* x, cudaStream_t s);
+static int exact_scratch_alloc(pct_ctx* c);
 static const int kGraphPairs = 64;
 // Upload chunks (histories): the first one is small so that the first DROP blocks start after about a
 // millisecond, the following ones double up to 2^24 (64 MB per float field) so that a 19 GB upload is
@@ -385,6 +389,7 @@ extern "C" void pct_destroy(pct_ctx* c) {
     if (c->tab) cudaFree(c->tab);
     if (c->ctrl) cudaFree(c->ctrl);
     if (c->wctrl) cudaFree(c->wctrl);
+    if (c->exact_scratch) cudaFree(c->exact_scratch);
     if (c->tvs_grad) cudaFree(c->tvs_grad);
     if (c->tvs_state) cudaFree(c->tvs_state);
     (void)cudaGetLastError();
@@ -566,6 +571,8 @@ static DropArgs drop_args(pct_ctx* c, long long block_size, long long first, lon
     a.tab = c->tab;
     a.ctrl = c->ctrl;
     a.order = first < 0 ? c->order : nullptr;
+    a.scratch = c->exact_scratch;
+    a.cap_lane = c->exact_cap;
     return a;
 }
 
@@ -721,7 +728,7 @@ extern "C" int pct_iterate(pct_ctx* c, float lambda, int64_t block_size, int n_i
     if (n_iter == 0) return PCT_OK;
     DeviceGuard guard(c->device);
     const bool tvs = c->tvs_beta0 > 0.0f;  // a step on the image that enters every block: launches go out one by one
-    if (c->engine == 1 && !tvs) return iterate_wave(c, lambda, block_size, n_iter);
+    if (c->engine == 1 && !tvs && !c->exact_scratch) return iterate_wave(c, lambda, block_size, n_iter);
     const long long n_blocks = (c->n + block_size - 1) / block_size;
     const long long pairs = n_blocks * (long long)n_iter;
     CUDA_TRY(c, cudaMemsetAsync(c->ctrl, 0, sizeof(Ctrl), c->stream));
@@ -813,12 +820,13 @@ extern "C" int pct_iterate_carp(pct_ctx* c, float lambda, int64_t block_size, in
         }
         c->carp_p = P;
     }
-    if (c->engine == 1) {
+    const bool wave = c->engine == 1 && !c->exact_scratch;
+    if (wave) {
         if (int rc = ensure_plans(c, block_size, P)) return rc;
     } else {
         prepare_order(c, block_size, P);
     }
-    if (c->engine != 1 && c->order && c->order_built == 0) {  // every string's blocks, ordered by depth slab (k_order_blocks)
+    if (!wave && c->order && c->order_built == 0) {  // every string's blocks, ordered by depth slab (k_order_blocks)
         for (int p = 0; p < P; ++p) {
             const long long lo = (long long)(((__int128)p * c->n) / P), hi = (long long)(((__int128)(p + 1) * c->n) / P);
             HistPtrs Hs = c->H;
@@ -838,7 +846,7 @@ extern "C" int pct_iterate_carp(pct_ctx* c, float lambda, int64_t block_size, in
             float* xs = c->carp_x + (size_t)p * stride;
             CUDA_TRY(c, cudaStreamWaitEvent(s, c->carp_fork, 0));
             CUDA_TRY(c, cudaMemcpyAsync(xs, c->x, sizeof(float) * M, cudaMemcpyDeviceToDevice, s));  // the common x0
-            if (c->engine == 1) {
+            if (wave) {
                 // every string gets its share of the CTA slots: P persistent launches side by side
                 const int grid_p = (c->wave_grid + P - 1) / P;
                 if (int rc = wave_sweep(c, c->plans[p], block_size, lambda, xs, c->carp_acc + (size_t)p * stride, c->carp_wctrl + p, grid_p, s, false))
@@ -855,6 +863,8 @@ extern "C" int pct_iterate_carp(pct_ctx* c, float lambda, int64_t block_size, in
             a.n = hi - lo;
             a.x = xs;
             a.acc = c->carp_acc + (size_t)p * stride;
+            if (a.scratch)  // exact-traversal mode: the strings' kernels run concurrently, each on its own part of the scratch
+                a.scratch = (float2*)((char*)a.scratch + (size_t)p * exact_scratch_bytes(c->g.kmax, (c->drop_grid + P - 1) / P, nullptr));
             a.ctrl = c->carp_ctrl + p;
             a.order = c->order ? c->order + lo : nullptr;
             const long long n_blocks = (a.n + block_size - 1) / block_size;
@@ -870,7 +880,7 @@ extern "C" int pct_iterate_carp(pct_ctx* c, float lambda, int64_t block_size, in
         }
         CUDA_TRY(c, launch_mean(c->x, c->carp_x, P, M, stride, c->stream));
         // pct_get_stats: the counters of the strings' sweeps, added up
-        if (c->engine == 1)
+        if (wave)
             CUDA_TRY(c, launch_sum_stats(c->wctrl->last, c->carp_wctrl[0].last, sizeof(WaveCtrl), P, c->stream));
         else
             CUDA_TRY(c, launch_sum_stats(c->ctrl->last, c->carp_ctrl[0].last, sizeof(Ctrl), P, c->stream));
@@ -959,7 +969,32 @@ extern "C" int pct_set_step(pct_ctx* c, int substeps) {
     c->g.kmax = kmax;
     c->g.inv_step = 1.0f / step;
     drop_graph(c);  // the cached graph holds the old geometry
+    if (c->exact_scratch) return exact_scratch_alloc(c);  // (sized by the segments a lane can own)
     return PCT_OK;
+}
+
+static int exact_scratch_alloc(pct_ctx* c) {
+    if (c->exact_scratch) cudaFree(c->exact_scratch);
+    c->exact_scratch = nullptr;
+    // (room for 64 CTAs more than the grid: the CARP strings run side by side on ceil(grid / P) CTAs each, each with a region of its own)
+    const size_t bytes = exact_scratch_bytes(c->g.kmax, c->drop_grid + 64, &c->exact_cap);
+    CUDA_TRY(c, cudaMalloc(&c->exact_scratch, bytes));
+    CUDA_TRY(c, exact_configure(c->g.kmax));
+    return PCT_OK;
+}
+
+extern "C" int pct_set_walk(pct_ctx* c, int mode) {
+    if (!c) return PCT_EINVAL;
+    if (mode != PCT_WALK_MIDPOINT && mode != PCT_WALK_EXACT) return fail(c, PCT_EINVAL, "pct_set_walk: unknown mode");
+    DeviceGuard guard(c->device);
+    CUDA_TRY(c, cudaStreamSynchronize(c->stream));
+    drop_graph(c);  // the cached graph holds the other mode's kernel
+    if (mode == PCT_WALK_MIDPOINT) {
+        if (c->exact_scratch) cudaFree(c->exact_scratch);
+        c->exact_scratch = nullptr;
+        return PCT_OK;
+    }
+    return exact_scratch_alloc(c);
 }
 
 extern "C" int pct_set_path_model(pct_ctx* c, int model) {
@@ -1015,11 +1050,13 @@ extern "C" int pct_get_stats(pct_ctx* c, int64_t out[4]) {
     if (!c || !out) return PCT_EINVAL;
     DeviceGuard guard(c->device);
     unsigned long long last[4] = {0, 0, 0, 0};
-    const void* src = c->engine == 1 ? (const void*)c->wctrl->last : (const void*)c->ctrl->last;
+    const void* src = (c->engine == 1 && !c->exact_scratch) ? (const void*)c->wctrl->last : (const void*)c->ctrl->last;
     CUDA_TRY(c, cudaMemcpyAsync(last, src, sizeof(last), cudaMemcpyDeviceToHost, c->stream));
     CUDA_TRY(c, cudaStreamSynchronize(c->stream));
     for (int i = 0; i < 3; ++i) out[i] = (int64_t)last[i];
     out[3] = c->n;
+    if (c->exact_scratch && last[3] > 0)
+        return fail(c, PCT_EINTERNAL, "exact traversal: a path produced more runs than a lane's scratch holds (slopes beyond any tracker's)");
     wave_prof_dump("pct_get_stats");
     bounds_dump("pct_get_stats");
     return check_wave_error(c);
@@ -1046,6 +1083,10 @@ extern "C" int pct_debug_rows(pct_ctx* c, int64_t first, int64_t count, int32_t 
     a.seg_len = seg_len; a.row_len = row_len; a.nodes = nodes;
     DeviceGuard guard(c->device);
     if (int rc = wait_upload(c, first + count)) return rc;
+    if (c->exact_scratch) {
+        CUDA_TRY(c, launch_rows_exact(a, c->sm_count, c->stream));
+        return PCT_OK;
+    }
     CUDA_TRY(c, launch_rows(a, c->stream));
     return PCT_OK;
 }
@@ -1059,7 +1100,7 @@ extern "C" int pct_debug_block(pct_ctx* c, int64_t first, int64_t count, float* 
     if (count > (1LL << 24)) return fail(c, PCT_EINVAL, "pct_debug_block: count must be <= 2^24 (hit counts are held exactly in fp32)");
     DeviceGuard guard(c->device);
     if (int rc = wait_upload(c, first + count)) return rc;
-    if (c->engine == 1) {  // the wavefront kernel in its plain mode: the range as ONE block in the caller's order, no update
+    if (c->engine == 1 && !c->exact_scratch) {  // the wavefront kernel in its plain mode: the range as ONE block in the caller's order, no update
         CUDA_TRY(c, cudaMemsetAsync(&c->wctrl->ticket, 0, sizeof(c->wctrl->ticket), c->stream));
         WaveArgs w = wave_args(c, nullptr, count, 1.0f, c->x, c->acc, c->wctrl, c->wave_grid);
         w.first = first;
@@ -1086,7 +1127,7 @@ extern "C" int pct_profile_sweep(pct_ctx* c, float lambda, int64_t block_size, f
     DeviceGuard guard(c->device);
     if (int rc = wait_upload(c, -1)) return rc;
     const long long n_blocks = (c->n + block_size - 1) / block_size;
-    if (c->engine == 1) {  // one persistent launch per sweep: its device time IS the sweep's
+    if (c->engine == 1 && !c->exact_scratch) {  // one persistent launch per sweep: its device time IS the sweep's
         if (int rc = ensure_plans(c, block_size, 0)) return rc;
         if (int rc = build_plan(c, c->plans[0], block_size, n_blocks, c->stream)) return rc;  // (the plan is made once per history set: not timed)
         cudaEvent_t e0 = nullptr, e1 = nullptr;

@@ -38,6 +38,8 @@ struct DropArgs {
     Ctrl* ctrl;
     const uint32_t* order; // block mode: order[b*block_size + r] = offset inside DROP block b of the r-th
                            // history to process (k_order_blocks); nullptr: the caller's order
+    float2* scratch;       // exact-traversal mode (pct_exact.cu): runs of every lane, cap_lane entries per lane; else nullptr
+    int cap_lane;
 };
 
 struct RowsArgs {
@@ -49,6 +51,12 @@ struct RowsArgs {
     int32_t *nseg, *nnz, *seg_idx;
     float *seg_len, *row_len, *nodes;
 };
+
+// exact-traversal mode (pct_exact.cu)
+size_t exact_scratch_bytes(int kmax, int grid, int* cap_lane_out);
+cudaError_t exact_configure(int kmax);
+cudaError_t launch_drop_exact(const DropArgs& a, int grid, cudaStream_t stream);
+cudaError_t launch_rows_exact(const RowsArgs& a, int sms, cudaStream_t stream);
 
 // launchers (pct_kernels.cu); all asynchronous on `stream`, return the launch error
 size_t drop_smem_bytes(int nmin);

@@ -243,6 +243,7 @@ static cudaError_t launch_pdl(void (*kernel)(KArgs...), dim3 grid, dim3 block, s
 }
 
 cudaError_t launch_drop_block(const DropArgs& a, int grid, cudaStream_t stream) {
+    if (a.scratch != nullptr) return launch_drop_exact(a, grid, stream);  // exact-traversal mode (pct_exact.cu)
     // never more warps than histories (small blocks: one history per warp)
     const long long cnt = a.first < 0 ? a.block_size : a.count;
     const long long need = (cnt + kWarpsPerCta - 1) / kWarpsPerCta;

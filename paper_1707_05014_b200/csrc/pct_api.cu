@@ -676,8 +676,13 @@ static int wave_sweep(pct_ctx* c, WavePlan& pl, long long block_size, float lamb
     CUDA_TRY(c, cudaMemsetAsync(ctrl->upd_seq, 0, 5 * sizeof(ctrl->upd_seq), s));
     CUDA_TRY(c, cudaMemsetAsync(pl.done, 0, sizeof(int) * (size_t)pl.n_blocks * c->shape.n_slabs, s));
     WaveArgs a = wave_args(c, &pl, block_size, lambda, x, acc, ctrl, grid);
+    long long seg = pl.n_blocks;  // blocks per launch (PCT_WAVE_SEG: a tuning knob; 1 = a kernel boundary after every block)
+    if (const char* env = getenv("PCT_WAVE_SEG")) {
+        const long long v = atoll(env);
+        if (v >= 1) seg = v;
+    }
     for (long long q = 0; q < pl.n_blocks;) {
-        long long q1 = pl.n_blocks;
+        long long q1 = q + seg < pl.n_blocks ? q + seg : pl.n_blocks;
         if (on_main) {
             if (c->chunks_waited < c->chunk_ev.size() && q + kGraphPairs < q1) q1 = q + kGraphPairs;
             if (int rc = wait_upload(c, q1 < pl.n_blocks ? pl.first + q1 * block_size : -1)) return rc;

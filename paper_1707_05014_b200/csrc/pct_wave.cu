@@ -62,7 +62,7 @@ constexpr int kUpdaters = PCT_WAVE_UPDATERS;
 constexpr int kWalkers = kWarpsPerCta - kUpdaters;
 constexpr int kStageGroups = 256;                // groups of four voxels staged at once by an updater warp
 constexpr int kStageBytes = kStageGroups * 48;   // 32 B of accumulator + 16 B of image per group
-static_assert(kUpdaters >= 1 && kWalkers >= 1, "a CTA needs both roles");
+static_assert(kUpdaters >= 0 && kWalkers >= 1, "a CTA needs walkers");  // (kUpdaters = 0: the walkers run the updates while they wait)
 
 __host__ __device__ inline int wave_stage_off(int nmin) { return (smem_layout(nmin).total + 15) & ~15; }
 static size_t wave_smem_bytes(int nmin) { return (size_t)wave_stage_off(nmin) + (size_t)kUpdaters * kStageBytes; }

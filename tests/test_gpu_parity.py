@@ -619,3 +619,14 @@ def test_carp_across_two_contexts_averaged_in_place_is_carp_with_two_strings(ora
     x_ref = oracle_mod.carp_iterate(geom, oracle_mod.Histories(H), lam, B, iters, 2, np.zeros(M))
     assert np.linalg.norm(got - x_ref) <= REL_L2_PER_ITER * np.linalg.norm(x_ref)
     assert np.abs(got - x_ref).max() <= ABS_FINAL
+
+
+@pytest.mark.parametrize("n_strings", [2, 3])
+def test_carp_on_an_odd_grid(oracle_mod, pct, torch_cuda, n_strings):
+    """CARP with several strings on the 45 x 71 x 5 grid (15975 voxels: not a multiple of four; the strings' images and
+    accumulators must each start on a 16-byte boundary, and the stored slices are padded to even sides)."""
+    base = synth.config(0)
+    cfg = synth.Config(9, "odd", 9000, 45, 71, 5, 0.8, 37, 500, 0.1, 1, base.shapes * 0.5, seed=99)
+    H = synth.generate_numpy(cfg, 9000)
+    x, x_ref = _carp_parity(oracle_mod, pct, torch_cuda, cfg, H, 0.5, 500, 2, n_strings)
+    assert np.linalg.norm(x_ref) > 0.5

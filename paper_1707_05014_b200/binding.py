@@ -194,9 +194,9 @@ def pct_debug_block(ctx, first, count, delta, cnt):
 
 def pct_profile_sweep(ctx, lam, block_size):
     """One sweep with CUDA events around every launch -> dict of device times (include/pct.h)."""
-    out = (C.c_float * 4)()
+    out = (C.c_float * 6)()
     _check(ctx, lib().pct_profile_sweep(ctx, float(lam), int(block_size), out))
-    return dict(accumulate_ms=out[0], update_ms=out[1], sweep_ms=out[2], blocks=int(out[3]))
+    return dict(accumulate_ms=out[0], update_ms=out[1], sweep_ms=out[2], blocks=int(out[3]), tvs_ms=out[4])
 
 
 def pct_measure_peaks(footprint_bytes, cuda_stream=None):

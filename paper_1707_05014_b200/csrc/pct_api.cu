@@ -1123,7 +1123,7 @@ extern "C" int pct_debug_block(pct_ctx* c, int64_t first, int64_t count, float* 
     return PCT_OK;
 }
 
-extern "C" int pct_profile_sweep(pct_ctx* c, float lambda, int64_t block_size, float out_ms[4]) {
+extern "C" int pct_profile_sweep(pct_ctx* c, float lambda, int64_t block_size, float out_ms[6]) {
     if (!c) return PCT_EINVAL;
     if (!out_ms) return fail(c, PCT_EINVAL, "pct_profile_sweep: out_ms is NULL");
     if (!c->have_hist) return fail(c, PCT_ESTATE, "pct_profile_sweep: no histories set");
@@ -1153,15 +1153,17 @@ extern "C" int pct_profile_sweep(pct_ctx* c, float lambda, int64_t block_size, f
         out_ms[1] = 0.f;
         out_ms[2] = ms;
         out_ms[3] = (float)launches;
+        out_ms[4] = out_ms[5] = 0.f;
         return check_wave_error(c);
     }
     const int kChunk = 256;  // blocks per batch of events
-    cudaEvent_t ev[2 * kChunk + 1];
+    cudaEvent_t ev[3 * kChunk + 1];  // per block: [TVS step] accumulate, update
     int made = 0;
     int rc = PCT_OK;
-    double drop_ms = 0.0, upd_ms = 0.0, total_ms = 0.0;
+    double drop_ms = 0.0, upd_ms = 0.0, tvs_ms = 0.0, total_ms = 0.0;
+    const bool tvs = c->tvs_beta0 > 0.0f;
     auto body = [&]() -> int {
-        for (; made < 2 * kChunk + 1; ++made) CUDA_TRY(c, cudaEventCreate(&ev[made]));
+        for (; made < 3 * kChunk + 1; ++made) CUDA_TRY(c, cudaEventCreate(&ev[made]));
         CUDA_TRY(c, cudaMemsetAsync(c->ctrl, 0, sizeof(Ctrl), c->stream));
         prepare_order(c, block_size);
         if (int rc2 = build_order(c, block_size, n_blocks)) return rc2;
@@ -1170,21 +1172,26 @@ extern "C" int pct_profile_sweep(pct_ctx* c, float lambda, int64_t block_size, f
             const int nb = (int)(n_blocks - b0 < kChunk ? n_blocks - b0 : kChunk);
             CUDA_TRY(c, cudaEventRecord(ev[0], c->stream));
             for (int i = 0; i < nb; ++i) {
+                if (tvs)
+                    if (int rc2 = tvs_step(c, c->x, c->stream)) return rc2;
+                CUDA_TRY(c, cudaEventRecord(ev[3 * i + 1], c->stream));
                 CUDA_TRY(c, launch_drop_block(a, c->drop_grid, c->stream));
-                CUDA_TRY(c, cudaEventRecord(ev[2 * i + 1], c->stream));
+                CUDA_TRY(c, cudaEventRecord(ev[3 * i + 2], c->stream));
                 CUDA_TRY(c, launch_update(c->x, c->acc, c->n_slots, lambda, c->ctrl, n_blocks, c->order != nullptr, c->stream));
-                CUDA_TRY(c, cudaEventRecord(ev[2 * i + 2], c->stream));
+                CUDA_TRY(c, cudaEventRecord(ev[3 * i + 3], c->stream));
             }
             CUDA_TRY(c, cudaStreamSynchronize(c->stream));
             for (int i = 0; i < nb; ++i) {
-                float d = 0.f, u = 0.f;
-                CUDA_TRY(c, cudaEventElapsedTime(&d, ev[2 * i], ev[2 * i + 1]));
-                CUDA_TRY(c, cudaEventElapsedTime(&u, ev[2 * i + 1], ev[2 * i + 2]));
+                float s = 0.f, d = 0.f, u = 0.f;
+                CUDA_TRY(c, cudaEventElapsedTime(&s, ev[3 * i], ev[3 * i + 1]));
+                CUDA_TRY(c, cudaEventElapsedTime(&d, ev[3 * i + 1], ev[3 * i + 2]));
+                CUDA_TRY(c, cudaEventElapsedTime(&u, ev[3 * i + 2], ev[3 * i + 3]));
+                tvs_ms += s;
                 drop_ms += d;
                 upd_ms += u;
             }
             float t = 0.f;
-            CUDA_TRY(c, cudaEventElapsedTime(&t, ev[0], ev[2 * nb]));
+            CUDA_TRY(c, cudaEventElapsedTime(&t, ev[0], ev[3 * nb]));
             total_ms += t;
         }
         return PCT_OK;
@@ -1195,6 +1202,8 @@ extern "C" int pct_profile_sweep(pct_ctx* c, float lambda, int64_t block_size, f
     out_ms[0] = (float)drop_ms;
     out_ms[1] = (float)upd_ms;
     out_ms[2] = (float)total_ms;
+    out_ms[4] = (float)tvs_ms;
+    out_ms[5] = 0.f;
     out_ms[3] = (float)n_blocks;
     return PCT_OK;
 }

@@ -36,7 +36,13 @@ __device__ __forceinline__ Nb forward(const float* __restrict__ a, const Geom& g
     return n;
 }
 
-__device__ __forceinline__ float term(const Nb& n) { return sqrtf(n.dx * n.dx + n.dy * n.dy + n.dz * n.dz + kTvEps2); }
+// t = sqrt(q) and 1 / t from one reciprocal square root (relative error 2^-22: far inside the step's tolerance)
+__device__ __forceinline__ float rterm(const Nb& n, float& t) {
+    const float q = n.dx * n.dx + n.dy * n.dy + n.dz * n.dz + kTvEps2;
+    const float r = rsqrtf(q);
+    t = q * r;
+    return r;
+}
 
 __device__ __forceinline__ double block_sum(double v, double* s_part) {
 #pragma unroll
@@ -60,35 +66,47 @@ __global__ void k_tv_reset(TvState* st) {
     for (int l = 0; l < kTvMaxLevels; ++l) st->tvz[l] = 0.0;
 }
 
-__global__ void __launch_bounds__(256) k_tv_grad(const float* __restrict__ x, float* __restrict__ grad, const Geom g, long long n_slots,
-                                                 TvState* st) {
+// Tile rows (one per CTA trip): entry q of tile row jt of a slice is voxel i = 2 (q >> 2) + (q & 1), j = 2 jt + ((q >> 1) & 1)
+// (voxel_slot read backwards, no division).
+__device__ __forceinline__ void tile_row_voxel(int q, int jt, int& i, int& j) {
+    i = ((q >> 2) << 1) + (q & 1);
+    j = 2 * jt + ((q >> 1) & 1);
+}
+
+__global__ void __launch_bounds__(256) k_tv_grad(const float* __restrict__ x, float* __restrict__ grad, const Geom g, TvState* st) {
     __shared__ double s_part[8];
     double tv = 0.0, g2 = 0.0;
-    const long long stride = (long long)gridDim.x * blockDim.x;
-    for (long long s = (long long)blockIdx.x * blockDim.x + threadIdx.x; s < n_slots; s += stride) {
-        int i, j, k;
-        voxel_of_slot((int)s, g.nxp, g.slice_p, i, j, k);
+    const int n_jt = g.slice_p / (2 * g.nxp), n_rows = n_jt * g.nz;
+    for (int row = blockIdx.x; row < n_rows; row += gridDim.x) {  // (a persistent grid: one block sum per CTA, not per row)
+    const int k = row / n_jt, jt = row - k * n_jt;
+    const long long row0 = (long long)k * g.slice_p + (long long)jt * 2 * g.nxp;
+    for (int q = threadIdx.x; q < 2 * g.nxp; q += blockDim.x) {
+        int i, j;
+        tile_row_voxel(q, jt, i, j);
         float gv = 0.0f;
         if (i < g.nx && j < g.ny) {  // (padding slots of odd grids hold nothing)
             const Nb n = forward(x, g, i, j, k);
-            const float t = term(n);
-            gv = -(n.dx + n.dy + n.dz) / t;  // d t_ijk / d x_ijk
-            if (i > 0) {                       // + d t_(i-1)jk / d x_ijk, ...
+            float t;
+            const float r = rterm(n, t);
+            gv = -(n.dx + n.dy + n.dz) * r;  // d t_ijk / d x_ijk
+            float tm;
+            if (i > 0) {                        // + d t_(i-1)jk / d x_ijk, ...
                 const Nb m = forward(x, g, i - 1, j, k);
-                gv += m.dx / term(m);
+                gv += m.dx * rterm(m, tm);
             }
             if (j > 0) {
                 const Nb m = forward(x, g, i, j - 1, k);
-                gv += m.dy / term(m);
+                gv += m.dy * rterm(m, tm);
             }
             if (k > 0) {
                 const Nb m = forward(x, g, i, j, k - 1);
-                gv += m.dz / term(m);
+                gv += m.dz * rterm(m, tm);
             }
             tv += (double)t;
             g2 += (double)gv * (double)gv;
         }
-        grad[s] = gv;
+        grad[row0 + q] = gv;
+    }
     }
     const double a = block_sum(tv, s_part);
     const double b = block_sum(g2, s_part);
@@ -98,8 +116,8 @@ __global__ void __launch_bounds__(256) k_tv_grad(const float* __restrict__ x, fl
     }
 }
 
-__global__ void __launch_bounds__(256) k_tv_probe(const float* __restrict__ x, const float* __restrict__ grad, const Geom g, long long n_slots,
-                                                  TvState* st, int parity, int n_half) {
+__global__ void __launch_bounds__(256) k_tv_probe(const float* __restrict__ x, const float* __restrict__ grad, const Geom g, TvState* st,
+                                                  int parity, int n_half) {
     __shared__ double s_part[8];
     const double g2 = st->g2;
     if (!(g2 > 0.0)) return;  // flat image: no direction, no step
@@ -107,10 +125,12 @@ __global__ void __launch_bounds__(256) k_tv_probe(const float* __restrict__ x, c
     double tz[kTvMaxLevels];
 #pragma unroll
     for (int l = 0; l < kTvMaxLevels; ++l) tz[l] = 0.0;
-    const long long stride = (long long)gridDim.x * blockDim.x;
-    for (long long s = (long long)blockIdx.x * blockDim.x + threadIdx.x; s < n_slots; s += stride) {
-        int i, j, k;
-        voxel_of_slot((int)s, g.nxp, g.slice_p, i, j, k);
+    const int n_jt = g.slice_p / (2 * g.nxp), n_rows = n_jt * g.nz;
+    for (int row = blockIdx.x; row < n_rows; row += gridDim.x) {
+    const int k = row / n_jt, jt = row - k * n_jt;
+    for (int q = threadIdx.x; q < 2 * g.nxp; q += blockDim.x) {
+        int i, j;
+        tile_row_voxel(q, jt, i, j);
         if (i >= g.nx || j >= g.ny) continue;
         const Nb a = forward(x, g, i, j, k), b = forward(grad, g, i, j, k);
         float sl = s0;
@@ -118,10 +138,12 @@ __global__ void __launch_bounds__(256) k_tv_probe(const float* __restrict__ x, c
         for (int l = 0; l < kTvMaxLevels; ++l) {
             if (l < n_half) {
                 const float dx = a.dx - sl * b.dx, dy = a.dy - sl * b.dy, dz = a.dz - sl * b.dz;
-                tz[l] += (double)sqrtf(dx * dx + dy * dy + dz * dz + kTvEps2);
+                const float q2 = dx * dx + dy * dy + dz * dz + kTvEps2;
+                tz[l] += (double)(q2 * rsqrtf(q2));
                 sl *= 0.5f;
             }
         }
+    }
     }
     for (int l = 0; l < n_half; ++l) {
         const double t = block_sum(tz[l], s_part);
@@ -162,9 +184,11 @@ cudaError_t launch_tvs_step(float* x, float* grad, const Geom& g, long long n_sl
     const long long cap = (long long)(sms > 0 ? sms : 148) * 8;
     if (blocks > cap) blocks = cap;
     if (blocks < 1) blocks = 1;
+    long long rows = (long long)(g.slice_p / (2 * g.nxp)) * g.nz;  // tile rows of the volume, dealt out to a persistent grid
+    if (rows > cap) rows = cap;
     k_tv_reset<<<1, 1, 0, stream>>>(st);
-    k_tv_grad<<<(int)blocks, 256, 0, stream>>>(x, grad, g, n_slots, st);
-    k_tv_probe<<<(int)blocks, 256, 0, stream>>>(x, grad, g, n_slots, st, parity, n_half);
+    k_tv_grad<<<(int)rows, 256, 0, stream>>>(x, grad, g, st);
+    k_tv_probe<<<(int)rows, 256, 0, stream>>>(x, grad, g, st, parity, n_half);
     k_tv_apply<<<(int)blocks, 256, 0, stream>>>(x, grad, n_slots, st, parity, n_half, gamma);
     return cudaGetLastError();
 }

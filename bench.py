@@ -389,8 +389,12 @@ def run_ours(args):
     }
     if "peaks_l2" in out:
         pk, pw = out["peaks_l2"], out["peaks_ws"]
-        rg, rr = pk["gather_path_tiled_per_s"], pk["red_v2_path_tiled_per_s"]
-        t_peak_hist = seg_per_hist / rg + nnz_per_hist / rr  # seconds per history at the measured L2 rates
+        rg, rr, rm = pk["gather_path_tiled_per_s"], pk["red_v2_path_tiled_per_s"], pk["mixed_pairs_tiled_per_s"]
+        # seconds per history at the measured L2 rates: the kernel's own mix (a gather and a reduction at the same voxel,
+        # measured together) for the non-zeros, plain gathers for the segments that continue a run; and, beside it, the
+        # two accesses at their separately measured rates, added up
+        t_peak_hist = nnz_per_hist / rm + (seg_per_hist - nnz_per_hist) / rg
+        t_peak_sum = seg_per_hist / rg + nnz_per_hist / rr
         l2_peak = l2_bytes / hist_per_launch / t_peak_hist / 1e9
         l2_ach = l2_bytes / t_kernel / 1e9
         alu_meas = pk["ffma_inst_per_s"] / 1e12
@@ -404,8 +408,10 @@ def run_ours(args):
                            "history = %.0f B/history x %d histories/launch" % (seg_per_hist, nnz_per_hist, l2_bytes / hist_per_launch,
                                                                                 hist_per_launch),
             "peak_source": "measured in this run, before the timed region (pct_measure_peaks, 32 MiB = L2-resident, accesses shaped like "
-                           "the row passes, voxels in the library's 2x2 tiles): %.0f G gathers/s, %.0f G reductions/s; peak = the same "
-                           "bytes at those rates" % (rg / 1e9, rr / 1e9),
+                           "the row passes, voxels in the library's 2x2 tiles): %.0f G (gather + reduction) pairs/s measured "
+                           "together, %.0f G gathers/s, %.0f G reductions/s alone; peak = the same bytes at the pair rate" % (
+                               rm / 1e9, rg / 1e9, rr / 1e9),
+            "frac_with_rates_added_up": (t_peak_sum * hist_per_launch) / t_kernel,
             "binds": max(times, key=times.get), "time_at_peak_us": times,
             "l2_rates_on_working_set": {"footprint_bytes": pw["footprint_bytes"],
                                         "gather_path_tiled_per_s": pw["gather_path_tiled_per_s"],

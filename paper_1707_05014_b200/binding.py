@@ -207,7 +207,7 @@ def pct_measure_peaks(footprint_bytes, cuda_stream=None):
         raise PctError(rc, "pct_measure_peaks failed")
     return dict(gather_random_per_s=out[0], gather_path_per_s=out[1], red_v2_random_per_s=out[2], stream_read_bytes_per_s=out[3],
                 ffma_inst_per_s=out[4], ffma2_inst_per_s=out[5], red_v2_path_per_s=out[6], footprint_bytes=int(out[7]),
-                gather_path_tiled_per_s=out[8], red_v2_path_tiled_per_s=out[9])
+                gather_path_tiled_per_s=out[8], red_v2_path_tiled_per_s=out[9], mixed_pairs_tiled_per_s=out[10])
 
 
 def pct_set_tvs(ctx, beta0, gamma=1.0, n_halvings=4):

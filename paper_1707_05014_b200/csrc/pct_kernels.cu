@@ -18,6 +18,7 @@
 #include <string.h>
 
 #include "pct_walk.cuh"
+#include "pct_walk16.cuh"
 
 namespace pct {
 
@@ -199,6 +200,137 @@ __global__ void __launch_bounds__(kThreads, kCtasPerSm) k_drop_block(const DropA
     }
 }
 
+// ---- two histories per warp (pct_walk16.cuh) --------------------------------------------------------------------
+// Shared memory: Sigma1^-1 table | PathState[warps][kBatch] | TWO row buffers per warp.
+__host__ __device__ inline SmemLayout smem_layout_pair(int kmax) {
+    SmemLayout l = smem_layout(kmax);
+    l.row_slots = row16_slots(kmax);
+    l.total = l.row_off + kWarpsPerCta * 2 * l.row_slots * (int)sizeof(float2);
+    return l;
+}
+size_t drop_pair_smem_bytes(int kmax) { return (size_t)smem_layout_pair(kmax).total; }
+
+// k_drop_block with the histories of an item walked two at a time, sixteen lanes each.  The item's histories are
+// sorted by their node count inside the warp first (a ten-step bitonic network on the keys the set-up lanes hold), so that
+// the two of a pair are about equally long: they share one chunk size.  Work queue, set-up, dependent launch and the
+// counters are those of k_drop_block.
+template <bool SPLINE>
+__global__ void __launch_bounds__(kThreads, kCtasPerSm) k_drop_pair(const DropArgs a) {
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    const Geom g = a.g;
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    const int hl = lane & 15, half = lane >> 4;
+    const SmemLayout lay = smem_layout_pair(g.kmax);
+    float4* s_tab = reinterpret_cast<float4*>(smem_raw);
+    PathState* s_state = reinterpret_cast<PathState*>(smem_raw + lay.state_off) + warp * kBatch;
+    float2* row = reinterpret_cast<float2*>(smem_raw + lay.row_off) + (warp * 2 + half) * lay.row_slots;  // this half's row buffer
+    __shared__ Queue q;
+    asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
+    stage_table(s_tab, a.tab, g.kmax);
+    asm volatile("griddepcontrol.wait;" ::: "memory");
+    if (threadIdx.x == 0) {
+        long long first = a.first, count = a.count;
+        if (first < 0) {
+            first = a.ctrl->block * a.block_size;
+            count = a.n - first < a.block_size ? a.n - first : a.block_size;
+        }
+        q = make_queue(first, count, (long long)gridDim.x * kWarpsPerCta);
+        q.interleave = a.first < 0 && a.order != nullptr;
+    }
+    __syncthreads();
+    unsigned long long rows = 0, nnz_total = 0, segs = 0;
+
+    const unsigned long long gw = (unsigned long long)blockIdx.x * kWarpsPerCta + warp;
+    for (bool first_item = true;; first_item = false) {
+        unsigned long long w = gw;
+        if (!first_item || gw >= q.n_static) {
+            if (lane == 0) w = q.n_static + atomicAdd(&a.ctrl->work, 1ULL);
+            w = __shfl_sync(0xffffffffu, w, 0);
+        }
+        if (w >= q.n_items) break;
+        long long rel0, stride;
+        int cnt;
+        queue_item(q, w, rel0, cnt, stride);
+        int myK = -1;
+        if (lane < cnt) {
+            long long r = rel0 + lane * stride;
+            if (q.interleave) r = (long long)__ldg(a.order + q.first + r);
+            PCT_BOUND(3, q.first + r >= 0 && q.first + r < a.n);
+            const Hist hh = load_history(a.H, q.first + r);
+            setup_history(g, hh, s_state[lane]);
+            myK = s_state[lane].K;
+        }
+        __syncwarp();
+        // the item's histories by node count (lanes 0-15 hold one each; kBatch <= 16): key = (K + 1) * 16 + slot, skipped
+        // histories and empty slots (K = -1) first; both halves sort the same keys
+        int key = __shfl_sync(0xffffffffu, myK, hl);
+        key = ((key + 1) << 4) | hl;
+        key = sort16(key, hl);
+        for (int p = 15; p >= 1; p -= 2) {  // pairs (p, p - 1) of the sorted order, longest first
+            const int ka = __shfl_sync(0xffffffffu, key, p), kb = __shfl_sync(0xffffffffu, key, p - 1);
+            const int Ka = (ka >> 4) - 1, Kb = (kb >> 4) - 1;  // Ka >= Kb
+            if (Ka < 0) break;                                  // nothing but skipped histories left
+            if (Kb < 0) {
+                // a history without a partner (odd item, or the partner was skipped): the whole warp walks it, 32 lanes,
+                // in the two row buffers taken as one
+                const PathState& S = s_state[ka & 15];
+                float2* row32 = reinterpret_cast<float2*>(smem_raw + lay.row_off) + warp * 2 * lay.row_slots;
+                float nrm;
+                int nnz;
+                const EmitPtrs no_emit{nullptr, nullptr, nullptr, nullptr};
+                walk_history<false, SPLINE>(g, S, s_tab, lane, row32, nrm, nnz, no_emit);
+                const int C = (Ka + 32) >> 5;
+                float dot = gather_row(row32, lane, C, a.x);
+                dot = warp_sum(dot);
+                nrm = warp_sum(nrm);
+                if (nrm > 0.0f) {
+                    const float r = __fdiv_rn(S.wepl - dot, nrm);
+                    scatter_row(row32, lane, C, a.acc, r);
+                    rows += (lane == 0);
+                    nnz_total += nnz;
+                }
+                if (lane == 0) segs += Ka + 1;
+                __syncwarp();
+                break;  // (everything below it in the sorted order is skipped)
+            }
+            const PathState& S = s_state[(half == 0 ? ka : kb) & 15];
+            const int C = (Ka + 16) >> 4;                       // chunk size of the pair: ceil((Ka + 1) / 16)
+            float nrm;
+            int nnz;
+            walk_history16<SPLINE>(g, S, s_tab, hl, C, row, nrm, nnz);
+            float dot = gather16_row(row, hl, C, a.x);
+            dot = half_sum(dot);
+            nrm = half_sum(nrm);
+            const bool live = nrm > 0.0f;                       // non-empty row (R13)
+            const float r = live ? __fdiv_rn(S.wepl - dot, nrm) : 0.0f;
+            scatter16_row(row, hl, C, a.acc, r, live);
+            if (hl == 0 && live) ++rows;
+            if (live) nnz_total += nnz;
+            if (hl == 0) segs += S.K + 1;
+            __syncwarp();  // the row buffers are reused by the next pair
+        }
+        __syncwarp();  // the state records are reused by the next item
+    }
+    nnz_total = (unsigned long long)__reduce_add_sync(0xffffffffu, (unsigned)nnz_total);
+    rows = (unsigned long long)__reduce_add_sync(0xffffffffu, (unsigned)rows);
+    segs = (unsigned long long)__reduce_add_sync(0xffffffffu, (unsigned)segs);
+    if (lane == 0) {
+        atomicAdd(&a.ctrl->cur[0], rows);
+        atomicAdd(&a.ctrl->cur[1], nnz_total);
+        atomicAdd(&a.ctrl->cur[2], segs);
+    }
+}
+
+// PCT_PAIR=0 selects the one-history-per-warp kernel (k_drop_block).
+static bool pair_enabled() {
+    static int on = -1;
+    if (on < 0) {
+        const char* env = getenv("PCT_PAIR");
+        on = (env && env[0] == '0') ? 0 : 1;
+    }
+    return on == 1;
+}
+
 cudaError_t drop_configure(int nmin, int* grid_out) {
     if (((nmin + 32) >> 5) > 64) return cudaErrorInvalidValue;
     const size_t smem = drop_smem_bytes(nmin);
@@ -208,7 +340,12 @@ cudaError_t drop_configure(int nmin, int* grid_out) {
     if ((e = cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev)) != cudaSuccess) return e;
     e = cudaFuncSetAttribute(k_drop_block<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (e == cudaSuccess) e = cudaFuncSetAttribute(k_drop_block<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-    if (e == cudaSuccess) e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, k_drop_block<false>, kThreads, smem);
+    const size_t smem2 = drop_pair_smem_bytes(nmin);
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(k_drop_pair<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem2);
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(k_drop_pair<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem2);
+    if (e == cudaSuccess)
+        e = pair_enabled() ? cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, k_drop_pair<false>, kThreads, smem2)
+                           : cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, k_drop_block<false>, kThreads, smem);
     if (e != cudaSuccess) return e;
     if (per_sm < 1) return cudaErrorLaunchOutOfResources;
     *grid_out = sms * per_sm;  // persistent: every CTA slot of the chip, work handed out dynamically
@@ -248,6 +385,14 @@ cudaError_t launch_drop_block(const DropArgs& a, int grid, cudaStream_t stream) 
     const long long cnt = a.first < 0 ? a.block_size : a.count;
     const long long need = (cnt + kWarpsPerCta - 1) / kWarpsPerCta;
     if (need < grid) grid = need < 1 ? 1 : (int)need;
+    // two histories per warp pay when a warp's items hold pairs: with fewer than four histories per warp in the block
+    // (items of one history) the one-history kernel is the faster one (configs[1]: 30.6 against 31.3 us per block)
+    if (pair_enabled() && cnt >= 4LL * grid * kWarpsPerCta) {
+        const size_t smem2 = drop_pair_smem_bytes(a.g.kmax);
+        cudaError_t e2 = a.g.path_model == 1 ? launch_pdl(k_drop_pair<true>, dim3(grid), dim3(kThreads), smem2, stream, a)
+                                             : launch_pdl(k_drop_pair<false>, dim3(grid), dim3(kThreads), smem2, stream, a);
+        return e2 != cudaSuccess ? e2 : cudaGetLastError();
+    }
     const size_t smem = drop_smem_bytes(a.g.kmax);
     cudaError_t e = a.g.path_model == 1 ? launch_pdl(k_drop_block<true>, dim3(grid), dim3(kThreads), smem, stream, a)
                                         : launch_pdl(k_drop_block<false>, dim3(grid), dim3(kThreads), smem, stream, a);

@@ -377,7 +377,7 @@ def run_ours(args):
            "peak_source": "MEASURED_PEAKS.json hbm_gbs (%s)" % peaks["source"], "algorithmic": "38 B/history",
            "time_at_peak_us": HBM_BYTES_PER_HISTORY * hist_per_launch / (peaks["hbm_gbs"] * 1e9) * 1e6}
     common = {
-        "kernel": "pct::k_drop_block (fused hull+MLP+walk+projection+scatter)",
+        "kernel": "pct::k_drop_pair (fused hull+MLP+walk+projection+scatter, two histories per warp; k_drop_block for blocks under four histories per warp)",
         "kernel_ms": k_ms, "launches_timed": prof["blocks"],
         "kernel_share_of_step": prof["accumulate_ms"] / prof["sweep_ms"],
         "update_kernel_ms": prof["update_ms"] / prof["blocks"],

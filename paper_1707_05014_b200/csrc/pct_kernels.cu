@@ -321,14 +321,16 @@ __global__ void __launch_bounds__(kThreads, kCtasPerSm) k_drop_pair(const DropAr
     }
 }
 
-// PCT_PAIR=0 selects the one-history-per-warp kernel (k_drop_block).
-static bool pair_enabled() {
+// PCT_PAIR=0 selects the one-history-per-warp kernel (k_drop_block) everywhere.  The pair kernel is used where two of its
+// CTAs fit the shared memory of an SM like k_drop_block's do (not with the half-voxel step on wide grids: two row buffers
+// per warp of twice the length).
+static bool pair_enabled(int kmax) {
     static int on = -1;
     if (on < 0) {
         const char* env = getenv("PCT_PAIR");
         on = (env && env[0] == '0') ? 0 : 1;
     }
-    return on == 1;
+    return on == 1 && 2 * (drop_pair_smem_bytes(kmax) + 1024) <= 227 * 1024;
 }
 
 cudaError_t drop_configure(int nmin, int* grid_out) {
@@ -344,7 +346,7 @@ cudaError_t drop_configure(int nmin, int* grid_out) {
     if (e == cudaSuccess) e = cudaFuncSetAttribute(k_drop_pair<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem2);
     if (e == cudaSuccess) e = cudaFuncSetAttribute(k_drop_pair<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem2);
     if (e == cudaSuccess)
-        e = pair_enabled() ? cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, k_drop_pair<false>, kThreads, smem2)
+        e = pair_enabled(nmin) ? cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, k_drop_pair<false>, kThreads, smem2)
                            : cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, k_drop_block<false>, kThreads, smem);
     if (e != cudaSuccess) return e;
     if (per_sm < 1) return cudaErrorLaunchOutOfResources;
@@ -387,7 +389,7 @@ cudaError_t launch_drop_block(const DropArgs& a, int grid, cudaStream_t stream) 
     if (need < grid) grid = need < 1 ? 1 : (int)need;
     // two histories per warp pay when a warp's items hold pairs: with fewer than four histories per warp in the block
     // (items of one history) the one-history kernel is the faster one (configs[1]: 30.6 against 31.3 us per block)
-    if (pair_enabled() && cnt >= 4LL * grid * kWarpsPerCta) {
+    if (pair_enabled(a.g.kmax) && cnt >= 4LL * grid * kWarpsPerCta) {
         const size_t smem2 = drop_pair_smem_bytes(a.g.kmax);
         cudaError_t e2 = a.g.path_model == 1 ? launch_pdl(k_drop_pair<true>, dim3(grid), dim3(kThreads), smem2, stream, a)
                                              : launch_pdl(k_drop_pair<false>, dim3(grid), dim3(kThreads), smem2, stream, a);

@@ -627,6 +627,85 @@ __global__ void __launch_bounds__(kThreads) k_rows(const RowsArgs a) {
     }
 }
 
+// inspection of the two-histories-per-warp walk (pct_walk16.cuh; PCT_ROWS_PAIR=1): histories (2 w, 2 w + 1) of the range
+// are walked side by side exactly as k_drop_pair walks a pair, and the rows are read back from the two row buffers.
+// Node positions are not written by this walk (they are k_rows's, the same node_pair code).
+template <bool SPLINE>
+__global__ void __launch_bounds__(kThreads) k_rows_pair(const RowsArgs a) {
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    const Geom g = a.g;
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    const int hl = lane & 15, half = lane >> 4;
+    const SmemLayout lay = smem_layout_pair(g.kmax);
+    float4* s_tab = reinterpret_cast<float4*>(smem_raw);
+    PathState* s_state = reinterpret_cast<PathState*>(smem_raw + lay.state_off) + warp * kBatch;
+    float2* row = reinterpret_cast<float2*>(smem_raw + lay.row_off) + (warp * 2 + half) * lay.row_slots;
+    stage_table(s_tab, a.tab, g.kmax);
+    const long long n_pairs = (a.count + 1) / 2;
+    for (long long pr = (long long)blockIdx.x * kWarpsPerCta + warp; pr < n_pairs; pr += (long long)gridDim.x * kWarpsPerCta) {
+        const long long r = 2 * pr + half;  // this half's history
+        const bool have = r < a.count;
+        if (hl == 0) {
+            s_state[half].K = -1;
+            if (have) {
+                const Hist hh = load_history(a.H, a.first + r);
+                setup_history(g, hh, s_state[half]);
+            }
+        }
+        __syncwarp();
+        const int Ka = s_state[0].K, Kb = s_state[1].K;
+        const int Kmax = Ka > Kb ? Ka : Kb;
+        int nnz_total = 0;
+        const int K = s_state[half].K;
+        if (Kmax >= 0) {
+            const PathState& S = s_state[K >= 0 ? half : (half ^ 1)];  // (a half without a path walks its partner's, muted)
+            const int C = (Kmax + 16) >> 4;
+            float nrm;
+            int nnz;
+            walk_history16<SPLINE>(g, S, s_tab, hl, C, row, nrm, nnz);
+            nnz_total = nnz;
+#pragma unroll
+            for (int o = 8; o > 0; o >>= 1) nnz_total += __shfl_xor_sync(0xffffffffu, nnz_total, o, 16);
+            if (have && K >= 0) {
+                int32_t* o_idx = a.seg_idx ? a.seg_idx + (size_t)r * a.max_seg : nullptr;
+                float* o_len = a.seg_len ? a.seg_len + (size_t)r * a.max_seg : nullptr;
+                float* o_row = a.row_len ? a.row_len + (size_t)r * a.max_seg : nullptr;
+                for (int k = hl; k <= K; k += 16) {
+                    const float2 e = row[row_slot(k)];
+                    int lin = __float_as_int(e.x);
+                    if (lin >= 0) {
+                        int vi, vj, vk;
+                        voxel_of_slot(lin, g.nxp, g.slice_p, vi, vj, vk);
+                        lin = vi + g.nx * (vj + g.ny * vk);
+                    }
+                    if (o_idx) o_idx[k] = lin;
+                    if (o_len) o_len[k] = fabsf(e.y);
+                    if (o_row) o_row[k] = __float_as_int(e.y) < 0 ? 1.0f : 0.0f;
+                }
+            }
+            __syncwarp();
+            if (have && K >= 0 && a.row_len && a.seg_idx && a.seg_len) {
+                int32_t* o_idx = a.seg_idx + (size_t)r * a.max_seg;
+                float* o_len = a.seg_len + (size_t)r * a.max_seg;
+                float* o_row = a.row_len + (size_t)r * a.max_seg;
+                for (int k = hl; k <= K; k += 16) {
+                    if (o_row[k] > 0.0f) {
+                        const int idx = o_idx[k];
+                        float lm = o_len[k];
+                        for (int m = k + 1; m <= K && o_idx[m] == idx; ++m) lm += o_len[m];
+                        o_row[k] = lm;
+                    }
+                }
+            }
+        }
+        if (hl == 0 && have) {
+            a.nseg[r] = K >= 0 ? K + 1 : 0;
+            a.nnz[r] = K >= 0 ? nnz_total : 0;
+        }
+        __syncwarp();
+    }
+}
+
 cudaError_t launch_rows(const RowsArgs& a, cudaStream_t stream) {
     if (((a.g.kmax + 32) >> 5) > 64) return cudaErrorInvalidValue;
     const size_t smem = drop_smem_bytes(a.g.kmax);
@@ -635,6 +714,18 @@ cudaError_t launch_rows(const RowsArgs& a, cudaStream_t stream) {
     if (blocks > cap) blocks = cap;
     if (blocks < 1) blocks = 1;
     cudaError_t e = cudaSuccess;
+    const char* env = getenv("PCT_ROWS_PAIR");
+    if (env && env[0] == '1' && a.nodes == nullptr && pair_enabled(a.g.kmax)) {  // the hot path's pair walk, inspected
+        const size_t smem2 = drop_pair_smem_bytes(a.g.kmax);
+        if (a.g.path_model == 1) {
+            e = cudaFuncSetAttribute(k_rows_pair<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem2);
+            if (e == cudaSuccess) k_rows_pair<true><<<(int)blocks, kThreads, smem2, stream>>>(a);
+        } else {
+            e = cudaFuncSetAttribute(k_rows_pair<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem2);
+            if (e == cudaSuccess) k_rows_pair<false><<<(int)blocks, kThreads, smem2, stream>>>(a);
+        }
+        return e != cudaSuccess ? e : cudaGetLastError();
+    }
     if (a.g.path_model == 1) {
         e = cudaFuncSetAttribute(k_rows<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
         if (e == cudaSuccess) k_rows<true><<<(int)blocks, kThreads, smem, stream>>>(a);

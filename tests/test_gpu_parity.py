@@ -630,3 +630,47 @@ def test_carp_on_an_odd_grid(oracle_mod, pct, torch_cuda, n_strings):
     H = synth.generate_numpy(cfg, 9000)
     x, x_ref = _carp_parity(oracle_mod, pct, torch_cuda, cfg, H, 0.5, 500, 2, n_strings)
     assert np.linalg.norm(x_ref) > 0.5
+
+
+@pytest.mark.parametrize("index,n", [(0, 6001), (3, 2500), (4, 1001)])
+def test_rows_of_the_pair_walk_bit_exact(oracle_mod, pct, torch_cuda, monkeypatch, index, n):
+    """The walk of the throughput kernel (k_drop_pair: two histories per warp, sixteen lanes each, one chunk size per
+    pair) inspected directly: PCT_ROWS_PAIR=1 makes pct_debug_rows walk histories (2w, 2w+1) side by side with that code.
+    Voxel sequences, segment lengths (bitwise) and merged rows against the oracle; odd counts leave a lone last history."""
+    monkeypatch.setenv("PCT_ROWS_PAIR", "1")
+    torch = torch_cuda
+    cfg = synth.config(index)
+    H = synth.generate_numpy(cfg, n)
+    geom = oracle_geom(oracle_mod, cfg)
+    hs = oracle_mod.Histories(H)
+    D = to_device(H)
+    ms = geom.nmin + 2
+    ctx = _ctx(pct, torch, cfg)
+    try:
+        pct.pct_set_histories(ctx, n, D)
+        nseg = torch.zeros(n, dtype=torch.int32, device="cuda")
+        nnz = torch.zeros(n, dtype=torch.int32, device="cuda")
+        seg_idx = torch.full((n, ms), -7, dtype=torch.int32, device="cuda")
+        seg_len = torch.zeros((n, ms), dtype=torch.float32, device="cuda")
+        row_len = torch.zeros((n, ms), dtype=torch.float32, device="cuda")
+        pct.pct_debug_rows(ctx, 0, n, ms, nseg, nnz, seg_idx, seg_len, row_len, None)  # (no nodes: the pair walk is used)
+        pct.pct_synchronize(ctx)
+        nseg, nnz, seg_idx, seg_len, row_len = (t.cpu().numpy() for t in (nseg, nnz, seg_idx, seg_len, row_len))
+    finally:
+        pct.pct_destroy(ctx)
+    table = oracle_mod.sigma1_table(geom.h, geom.nmin)
+    paths = 0
+    for i in range(n):
+        r = oracle_mod.row_f32(geom, hs.hist(i), table)
+        ns = r["nseg"]
+        assert nseg[i] == ns and nnz[i] == r["nnz"], i
+        if ns == 0:
+            continue
+        paths += 1
+        assert np.array_equal(seg_idx[i, :ns], r["seg_idx"]), i
+        inside = r["seg_idx"] >= 0  # (the row buffer of the hot path keeps no length for a segment outside the grid)
+        assert np.array_equal(seg_len[i, :ns][inside], r["seg_len"][inside]), i
+        heads = row_len[i, :ns] > 0
+        assert np.array_equal(seg_idx[i, :ns][heads], r["row_idx"]), i
+        assert row_len[i, :ns][heads] == pytest.approx(r["row_len"], rel=1e-6)
+    assert paths > n // 2

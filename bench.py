@@ -9,11 +9,16 @@ Contract (driver): ``python bench.py --gpus N --steps K --warmup W`` prints ONE 
     iteration of the paper's solver; `value` = N / step time = protons*iterations/s.
   * `value`: histories resident in HBM; `e2e`: the same step through the C ABI from pinned HOST
     arrays (pct_set_histories_host -> pct_iterate -> pct_get_image to host), copies inside the timing.
-  * `roofline`: the fused accumulate kernel, timed with CUDA events around every launch
-    (pct_profile_sweep); `cpu_baseline`: the oracle timed on this box's host cores on a bounded sample.
+  * `roofline`: the fused accumulate kernel, timed with CUDA events around every launch (pct_profile_sweep), against the
+    L2 rate measured in this run for its own access mix (pct_measure_peaks: 4 B gathers + 8 B vector reductions shaped like
+    the row passes, L2-resident footprint) -- the metric's "HBM/L2 roofline"; the fp32-issue and HBM figures are reported
+    beside it (`roofline.alu`, `roofline.hbm`), `roofline.traffic` comes from the ncu captures named in profiles/traffic.json;
+    `cpu_baseline`: the oracle timed on this box's host cores on a bounded sample.
   * ``--impl reference``: the oracle as it stands on the host cores (there is no reference code).
   * N > 1 (torchrun): replicas only -- every rank runs the same workload on its own histories, no
     data-path collective; value = sum of histories / max time.
+  * side measurements (short JSON lines, not the driver's contract): --peaks, --carp (CARP, one string per rank under
+    torchrun), --carp-strings P, --time-ordered, --path-model spline.
 Inputs are seeded synthetic histories (synth/), generated on the GPU; nothing reads /root/reference.
 """
 import argparse

@@ -12,7 +12,7 @@ Contract (driver): ``python bench.py --gpus N --steps K --warmup W`` prints ONE 
   * `roofline`: the fused accumulate kernel, timed with CUDA events around every launch (pct_profile_sweep), against the
     L2 rate measured in this run for its own access mix (pct_measure_peaks: 4 B gathers + 8 B vector reductions shaped like
     the row passes, L2-resident footprint) -- the metric's "HBM/L2 roofline"; the fp32-issue and HBM figures are reported
-    beside it (`roofline.alu`, `roofline.hbm`), `roofline.traffic` comes from the ncu captures named in profiles/traffic.json;
+    beside it (`roofline.alu`, `roofline.hbm`), `roofline.traffic` comes from the ncu captures named in profiles/traffic.csv;
     `cpu_baseline`: the oracle timed on this box's host cores on a bounded sample.
   * ``--impl reference``: the oracle as it stands on the host cores (there is no reference code).
   * N > 1 (torchrun): replicas only -- every rank runs the same workload on its own histories, no
@@ -43,18 +43,24 @@ OPS_PER_SEGMENT = 106
 HBM_BYTES_PER_HISTORY = 38
 SM_COUNT = 148
 LANES_PER_SM = 128
-# dram__bytes_read.sum + dram__bytes_write.sum of ONE k_drop_block launch come from the committed ncu captures of
-# THIS build, recorded in profiles/traffic.json (file, commit, bytes per launch with ncu's cache flush and with
+# dram__bytes_read.sum + dram__bytes_write.sum of ONE launch of the fused accumulate kernel come from the committed ncu
+# captures of THIS build, recorded in profiles/traffic.csv (file, commit, bytes per launch with ncu's cache flush and with
 # --cache-control none), keyed by "config:block_size".
-TRAFFIC_JSON = os.path.join(ROOT, "profiles", "traffic.json")
+TRAFFIC_CSV = os.path.join(ROOT, "profiles", "traffic.csv")
 
 
 def ncu_traffic(config, block_size):
     try:
-        with open(TRAFFIC_JSON) as f:
-            return json.load(f).get("%d:%d" % (config, block_size))
-    except (OSError, ValueError):
-        return None
+        import csv
+
+        with open(TRAFFIC_CSV) as f:
+            for row in csv.DictReader(f):
+                if row["config:block_size"] == "%d:%d" % (config, block_size):
+                    return {"cold_bytes": float(row["cold_bytes"]), "warm_bytes": float(row["warm_bytes"]), "commit": row["commit"],
+                            "file": row["file"], "kernel": row["kernel"]}
+    except (OSError, ValueError, KeyError):
+        pass
+    return None
 
 
 def parse_args():

@@ -136,9 +136,12 @@ cudaError_t launch_plan_blocks(const HistPtrs& H, const Geom& g, long long n, lo
 
 // ---- total-variation superiorization (pct_tvs.cu) ---------------------------------------------------------------
 constexpr int kTvMaxLevels = 8;
-struct TvState {
-    double tvx, g2;              // TV(x) and ||grad TV(x)||^2 of the step in progress
+struct TvSums {
+    double tvx, g2;              // TV(x) and ||grad TV(x)||^2
     double tvz[kTvMaxLevels];    // TV(x + beta 2^-l v)
+};
+struct TvState {
+    TvSums sums[2];              // sums[parity] of the step in progress; the step zeroes the other pair for the next one
     double tv_before, tv_after;  // of the last completed step
     float beta[2];               // beta[parity]: step size of the step in progress; the other slot receives the next one
     float beta_used;             // step of the last completed step (beta 2^-level, or beta 2^-n_half if none was accepted)

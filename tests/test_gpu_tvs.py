@@ -19,7 +19,7 @@ def _ctx(pct, torch, nx, ny, nz, h=1.0):
     return pct.pct_create(nx, ny, nz, h, -r - 10.0, r + 10.0, torch.cuda.current_stream().cuda_stream)
 
 
-@pytest.mark.parametrize("shape,beta,levels", [((64, 64, 8), 2.0, 4), ((45, 71, 5), 0.5, 3), ((128, 128, 32), 500.0, 8), ((16, 16, 1), 0.3, 2)])
+@pytest.mark.parametrize("shape,beta,levels", [((64, 64, 8), 2.0, 4), ((45, 71, 5), 0.5, 3), ((128, 128, 32), 500.0, 8), ((16, 16, 1), 0.3, 2), ((33, 20, 3), 0.4, 1), ((70, 66, 9), 50.0, 5)])
 def test_single_steps_against_the_oracle(shape, beta, levels):
     import torch
 

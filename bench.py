@@ -86,6 +86,9 @@ def parse_args():
     ap.add_argument("--cpu-seconds", type=float, default=15.0, help="target CPU time of the oracle sample")
     ap.add_argument("--path-model", default="mlp", choices=["mlp", "spline"],
                     help="spline: the cubic-spline path model (SURVEY.md 8(f) NEXT-3), a side measurement; the metric's is mlp")
+    ap.add_argument("--tvs", type=float, default=0.0, metavar="BETA",
+                    help="BETA > 0: a total-variation superiorization step (pct_set_tvs(BETA, 1.0, 4)) on the image that enters every "
+                         "block (PAPER.md:113; SURVEY.md 8(f) NEXT-2), a side measurement: four more launches per block")
     ap.add_argument("--carp-strings", type=int, default=0,
                     help="P > 0: time pct_iterate_carp with P strings instead of the metric's DROP sweep (SURVEY.md 8(f) NEXT-1; "
                          "a side measurement: one short JSON line, not the driver's contract)")
@@ -273,6 +276,8 @@ def run_ours(args):
         ctx = pct.pct_create(cfg.nx, cfg.ny, cfg.nz, cfg.h, cfg.u_in, cfg.u_out, stream.cuda_stream)
         try:
             pct.pct_set_path_model(ctx, pct.PCT_PATH_SPLINE if args.path_model == "spline" else pct.PCT_PATH_MLP)
+            if args.tvs > 0:
+                pct.pct_set_tvs(ctx, args.tvs, 1.0, 4)
             pct.pct_set_histories(ctx, n, P)
             for _ in range(args.warmup):
                 pct.pct_iterate(ctx, lam, B, 1)
@@ -291,6 +296,8 @@ def run_ours(args):
             out["ms_per_step"] = ms / args.steps
             out["clocks"] = clk.summary()
             out["stats"] = pct.pct_get_stats(ctx)
+            if args.tvs > 0:
+                out["tvs_state"] = pct.pct_get_tvs_state(ctx)
             # the dominant kernel, CUDA events around every launch, one more sweep of the same workload
             prof = pct.pct_profile_sweep(ctx, lam, B)
             out["prof"] = prof
@@ -315,6 +322,8 @@ def run_ours(args):
             ctx = pct.pct_create(cfg.nx, cfg.ny, cfg.nz, cfg.h, cfg.u_in, cfg.u_out, stream.cuda_stream)
             try:
                 pct.pct_set_path_model(ctx, pct.PCT_PATH_SPLINE if args.path_model == "spline" else pct.PCT_PATH_MLP)
+                if args.tvs > 0:
+                    pct.pct_set_tvs(ctx, args.tvs, 1.0, 4)
                 host_ms = [0.0, 0.0, 0.0]  # host clock: upload enqueue (+ device allocation), sweep enqueue, wait + D2H
 
                 def e2e_step():
@@ -449,12 +458,15 @@ def run_ours(args):
                    else "angles interleaved (every block sees every angle)",
                    "path_model": "most-likely path (the metric's)" if args.path_model == "mlp"
                    else "cubic spline (side measurement, SURVEY.md 8(f) NEXT-3; the roofline's op count is the MLP's)"},
-        "clocks": out["clocks"], "gpu_launches": 2 * n_blocks * args.steps,
+        "clocks": out["clocks"], "gpu_launches": (6 if args.tvs > 0 else 2) * n_blocks * args.steps,
         "segments_per_history": seg_per_hist, "nonzeros_per_history": nnz_per_hist,
         "skipped_fraction": 1.0 - st["rows"] / max(1, st["histories"]),
         "image_finite": out["image_finite"], "image_mean_central": out["image_mean_central"],
         "roofline": roofline,
     }
+    if args.tvs > 0:
+        line["config"]["tvs"] = "a TVS step before every block (side measurement): beta0 %g, gamma 1, 4 halvings" % args.tvs
+        line["tvs"] = {"us_per_step": 1e3 * out["prof"]["tvs_ms"] / max(1, out["prof"]["blocks"]), "state": out["tvs_state"]}
     if "e2e" in out:
         line["e2e"] = out["e2e"]
     if cpu is not None:

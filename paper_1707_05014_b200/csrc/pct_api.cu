@@ -69,6 +69,10 @@ struct pct_ctx {
     std::vector<cudaStream_t> carp_stream;
     std::vector<cudaEvent_t> carp_done;
     cudaEvent_t carp_fork = nullptr;
+    std::vector<cudaGraphExec_t> carp_graph;  // per string: kGraphPairs (accumulate, update) pairs, like `graph`
+    float carp_graph_lambda = 0.f;
+    long long carp_graph_block = 0, carp_graph_n = 0;
+    const void *carp_graph_hist_key = nullptr, *carp_graph_order = nullptr, *carp_graph_scratch = nullptr;
     // 0: the block engine (two launches per DROP block, replayed from a CUDA graph): the default, the faster one at
     // every config measured; 1: the wavefront engine (pct_wave.cu, one persistent launch per sweep), PCT_ENGINE=wave
     int engine = 0;
@@ -172,6 +176,9 @@ static void drop_graph(pct_ctx* c) {
         cudaGraphExecDestroy(c->graph);
         c->graph = nullptr;
     }
+    for (cudaGraphExec_t g : c->carp_graph)
+        if (g) cudaGraphExecDestroy(g);
+    c->carp_graph.clear();
 }
 
 // Make the compute stream wait for the upload of histories [0, upto) (all of them: upto < 0).
@@ -357,6 +364,9 @@ extern "C" int pct_create(pct_ctx** out, int nx, int ny, int nz, float h, float 
 }
 
 static void release_carp(pct_ctx* c) {
+    for (cudaGraphExec_t g : c->carp_graph)  // (they hold the strings' buffers)
+        if (g) cudaGraphExecDestroy(g);
+    c->carp_graph.clear();
     for (cudaStream_t s : c->carp_stream) {
         cudaStreamSynchronize(s);
         cudaStreamDestroy(s);
@@ -576,9 +586,29 @@ static DropArgs drop_args(pct_ctx* c, long long block_size, long long first, lon
     return a;
 }
 
-static int enqueue_pair(pct_ctx* c, const DropArgs& a, float lambda, long long n_blocks, cudaStream_t s) {
-    CUDA_TRY(c, launch_drop_block(a, c->drop_grid, s));
-    CUDA_TRY(c, launch_update(c->x, c->acc, c->n_slots, lambda, c->ctrl, n_blocks, c->order != nullptr, s));
+// One DROP block: accumulate over the block a.ctrl->block points at, then update a.x and advance the block index.
+static int enqueue_pair(pct_ctx* c, const DropArgs& a, int grid, float lambda, long long n_blocks, cudaStream_t s) {
+    CUDA_TRY(c, launch_drop_block(a, grid, s));
+    CUDA_TRY(c, launch_update(const_cast<float*>(a.x), a.acc, c->n_slots, lambda, a.ctrl, n_blocks, c->order != nullptr, s));
+    return PCT_OK;
+}
+
+// kGraphPairs such pairs as one executable graph (the block index lives on the device, so one graph serves every block).
+static int capture_pairs(pct_ctx* c, const DropArgs& a, int grid, float lambda, long long n_blocks, cudaGraphExec_t* out) {
+    cudaStream_t cap = nullptr;
+    CUDA_TRY(c, cudaStreamCreateWithFlags(&cap, cudaStreamNonBlocking));
+    cudaGraph_t gr = nullptr;
+    int rc = PCT_OK;
+    cudaError_t e = cudaStreamBeginCapture(cap, cudaStreamCaptureModeThreadLocal);
+    if (e == cudaSuccess) {
+        for (int i = 0; i < kGraphPairs && rc == PCT_OK; ++i) rc = enqueue_pair(c, a, grid, lambda, n_blocks, cap);
+        e = cudaStreamEndCapture(cap, &gr);
+    }
+    if (e == cudaSuccess && rc == PCT_OK) e = cudaGraphInstantiate(out, gr, 0);
+    if (gr) cudaGraphDestroy(gr);
+    cudaStreamDestroy(cap);
+    if (rc != PCT_OK) return rc;
+    CUDA_TRY(c, e);
     return PCT_OK;
 }
 
@@ -749,20 +779,7 @@ extern "C" int pct_iterate(pct_ctx* c, float lambda, int64_t block_size, int n_i
                            c->graph_hist_key == (const void*)c->H.t_in && c->graph_order == (const void*)c->order;
         if (!reuse) {
             drop_graph(c);
-            cudaStream_t cap = nullptr;
-            CUDA_TRY(c, cudaStreamCreateWithFlags(&cap, cudaStreamNonBlocking));
-            cudaGraph_t gr = nullptr;
-            int rc = PCT_OK;
-            cudaError_t e = cudaStreamBeginCapture(cap, cudaStreamCaptureModeThreadLocal);
-            if (e == cudaSuccess) {
-                for (int i = 0; i < kGraphPairs && rc == PCT_OK; ++i) rc = enqueue_pair(c, a, lambda, n_blocks, cap);
-                e = cudaStreamEndCapture(cap, &gr);
-            }
-            if (e == cudaSuccess && rc == PCT_OK) e = cudaGraphInstantiate(&c->graph, gr, 0);
-            if (gr) cudaGraphDestroy(gr);
-            cudaStreamDestroy(cap);
-            if (rc != PCT_OK) return rc;
-            CUDA_TRY(c, e);
+            if (int rc = capture_pairs(c, a, c->drop_grid, lambda, n_blocks, &c->graph)) return rc;
             c->graph_lambda = lambda;
             c->graph_block = block_size;
             c->graph_n = c->n;
@@ -781,7 +798,7 @@ extern "C" int pct_iterate(pct_ctx* c, float lambda, int64_t block_size, int n_i
         int rc = wait_upload(c, done < n_blocks ? (done + 1) * block_size : -1);
         if (rc == PCT_OK) rc = build_order(c, block_size, done < n_blocks ? done + 1 : n_blocks);
         if (rc == PCT_OK && tvs) rc = tvs_step(c, c->x, c->stream);
-        if (rc == PCT_OK) rc = enqueue_pair(c, a, lambda, n_blocks, c->stream);
+        if (rc == PCT_OK) rc = enqueue_pair(c, a, c->drop_grid, lambda, n_blocks, c->stream);
         if (rc) return rc;
     }
     return PCT_OK;
@@ -841,6 +858,22 @@ extern "C" int pct_iterate_carp(pct_ctx* c, float lambda, int64_t block_size, in
         }
         c->order_built = 1;
     }
+    {  // the strings' cached graphs hold these arguments
+        const bool same = c->carp_graph_lambda == lambda && c->carp_graph_block == block_size && c->carp_graph_n == c->n &&
+                          c->carp_graph_hist_key == (const void*)c->H.t_in && c->carp_graph_order == (const void*)c->order &&
+                          c->carp_graph_scratch == (const void*)c->exact_scratch && (int)c->carp_graph.size() == P;
+        if (!same) {
+            for (cudaGraphExec_t g : c->carp_graph)
+                if (g) cudaGraphExecDestroy(g);
+            c->carp_graph.assign(P, nullptr);
+            c->carp_graph_lambda = lambda;
+            c->carp_graph_block = block_size;
+            c->carp_graph_n = c->n;
+            c->carp_graph_hist_key = (const void*)c->H.t_in;
+            c->carp_graph_order = (const void*)c->order;
+            c->carp_graph_scratch = (const void*)c->exact_scratch;
+        }
+    }
     for (int it = 0; it < n_iter; ++it) {
         if (c->tvs_beta0 > 0.0f)  // "In CARP, TVS is applied just once to the initial solution at the start of each iteration"
             if (int rc = tvs_step(c, c->x, c->stream)) return rc;
@@ -876,10 +909,15 @@ extern "C" int pct_iterate_carp(pct_ctx* c, float lambda, int64_t block_size, in
             // every string gets its share of the CTA slots: P block launches in flight side by side, each P times
             // longer (measured at 256 x 256 x 128, 1e8 histories: the same rate as whole-grid launches, 5.4e8 /s)
             const int grid = (c->drop_grid + P - 1) / P;
-            for (long long b = 0; b < n_blocks; ++b) {
-                CUDA_TRY(c, launch_drop_block(a, grid, s));
-                CUDA_TRY(c, launch_update(xs, a.acc, M, lambda, a.ctrl, n_blocks, c->order != nullptr, s));
+            long long b = 0;
+            if (n_blocks >= 2 * kGraphPairs) {  // the string's block loop from a graph of its own, as in pct_iterate
+                if ((int)c->carp_graph.size() != P) c->carp_graph.assign(P, nullptr);
+                if (!c->carp_graph[p])
+                    if (int rc = capture_pairs(c, a, grid, lambda, n_blocks, &c->carp_graph[p])) return rc;
+                for (; b + kGraphPairs <= n_blocks; b += kGraphPairs) CUDA_TRY(c, cudaGraphLaunch(c->carp_graph[p], s));
             }
+            for (; b < n_blocks; ++b)
+                if (int rc = enqueue_pair(c, a, grid, lambda, n_blocks, s)) return rc;
             CUDA_TRY(c, cudaEventRecord(c->carp_done[p], s));
             CUDA_TRY(c, cudaStreamWaitEvent(c->stream, c->carp_done[p], 0));
         }

@@ -19,7 +19,8 @@ def _ctx(pct, torch, nx, ny, nz, h=1.0):
     return pct.pct_create(nx, ny, nz, h, -r - 10.0, r + 10.0, torch.cuda.current_stream().cuda_stream)
 
 
-@pytest.mark.parametrize("shape,beta,levels", [((64, 64, 8), 2.0, 4), ((45, 71, 5), 0.5, 3), ((128, 128, 32), 500.0, 8), ((16, 16, 1), 0.3, 2), ((33, 20, 3), 0.4, 1), ((70, 66, 9), 50.0, 5)])
+@pytest.mark.parametrize("shape,beta,levels", [((64, 64, 8), 2.0, 4), ((45, 71, 5), 0.5, 3), ((128, 128, 32), 500.0, 8), ((16, 16, 1), 0.3, 2), ((33, 20, 3), 0.4, 1), ((70, 66, 9), 50.0, 5),
+                                               ((256, 256, 128), 30.0, 4)])  # the last: the grid of configs[3] in full
 def test_single_steps_against_the_oracle(shape, beta, levels):
     import torch
 
@@ -63,7 +64,10 @@ def test_single_steps_against_the_oracle(shape, beta, levels):
             if info["level"] >= 0:  # the step has length beta_used in the 2-norm
                 assert np.linalg.norm(g - xr) == pytest.approx(info["beta_used"], rel=1e-3)
                 accepted += 1
-            xr, b = xr_new, 0.7 * info["beta_used"]
+            # The direction d / |d| of a term is ill-conditioned where the image has become locally flat (after a few steps
+            # |d| reaches 1e-5 at some of 8.4e6 voxels, and the fp32 rounding of x, 6e-8, turns it by 1e-3): on the full-size
+            # grid every step is compared on its own, the oracle restarting from the library's image.
+            xr, b = (g if M > 1_000_000 else xr_new), 0.7 * info["beta_used"]
         assert accepted >= 2 and st["accepted"] == accepted
         pct.pct_set_tvs(ctx, 0.0, 1.0, 1)  # off again
         with pytest.raises(pct.PctError):

@@ -56,7 +56,10 @@ static int sm_count() {
 #ifndef PCT_QUEUE_DIV
 #define PCT_QUEUE_DIV 2  // static items: 1/DIV of a warp's fair share of the block
 #endif
-constexpr int kPhases = 4;
+#ifndef PCT_QUEUE_PHASES
+#define PCT_QUEUE_PHASES 4
+#endif
+constexpr int kPhases = PCT_QUEUE_PHASES;
 struct Queue {
     long long first, count;
     int size[kPhases];                  // histories per item

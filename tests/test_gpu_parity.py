@@ -281,6 +281,18 @@ def test_carp_config0(oracle_mod, pct, torch_cuda, n_strings):
     assert np.linalg.norm(x_ref) > 1.0
 
 
+@pytest.mark.parametrize("n_strings", [2, 3])
+def test_carp_strings_long_enough_for_the_graph_loop(oracle_mod, pct, torch_cuda, n_strings):
+    """Strings of 150+ blocks: pct_iterate_carp replays every string's block loop from a CUDA graph of 64 (accumulate,
+    update) pairs (from 128 blocks per string on) and launches the ragged rest one by one; the second call reuses the
+    graphs.  Same comparison as the short strings."""
+    cfg = synth.config(0)
+    H = synth.generate_numpy(cfg, 60_011)
+    block = 200 if n_strings == 2 else 130  # 151 / 154 blocks per string, the last one ragged
+    x, x_ref = _carp_parity(oracle_mod, pct, torch_cuda, cfg, H, 0.5, block, 2, n_strings)
+    assert np.linalg.norm(x_ref) > 1.0
+
+
 @pytest.mark.parametrize("order", ["1", "2"])
 def test_carp_config1_sample_from_an_image(oracle_mod, pct, torch_cuda, monkeypatch, order):
     """configs[1] geometry and block size, 3 strings of 1e5 histories, two iterations from a non-trivial image;

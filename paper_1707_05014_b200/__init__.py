@@ -9,6 +9,7 @@ from .binding import (  # noqa: F401
     FIELDS,
     PCT_PATH_MLP,
     PCT_PATH_SPLINE,
+    PCT_TVS_STATIC_MAX_SLOTS,
     PCT_WALK_EXACT,
     PCT_WALK_MIDPOINT,
     PctError,
@@ -35,5 +36,6 @@ from .binding import (  # noqa: F401
     pct_set_walk,
     pct_synchronize,
     pct_tvs_step,
+    pct_tvs_step_static,
     pct_version,
 )

@@ -76,6 +76,8 @@ def lib():
         L.pct_image_storage.argtypes = [vp, C.POINTER(vp), C.POINTER(i64)]
         L.pct_tvs_step.argtypes = [vp]
         L.pct_get_tvs_state.argtypes = [vp, C.POINTER(C.c_double)]
+        L.pct_tvs_step_static.argtypes = [vp, C.c_int, C.c_int, C.c_int, C.c_float, C.c_int, vp, vp]
+        L.pct_tvs_step_static_error.restype = C.c_char_p
         _lib = L
     return _lib
 
@@ -83,7 +85,7 @@ def lib():
 EXPORTS = ("pct_create", "pct_set_histories", "pct_set_histories_host", "pct_set_histories_xyz", "pct_iterate", "pct_iterate_carp", "pct_set_path_model", "pct_get_image",
            "pct_set_image", "pct_synchronize", "pct_get_stats", "pct_destroy", "pct_last_error", "pct_version",
            "pct_debug_rows", "pct_debug_block", "pct_profile_sweep", "pct_measure_peaks", "pct_set_tvs", "pct_tvs_step", "pct_set_step", "pct_set_walk", "pct_image_storage",
-           "pct_get_tvs_state")
+           "pct_get_tvs_state", "pct_tvs_step_static", "pct_tvs_step_static_error")
 
 
 def _ptr(a):
@@ -223,6 +225,21 @@ def pct_get_tvs_state(ctx):
     out = (C.c_double * 6)()
     _check(ctx, lib().pct_get_tvs_state(ctx, out))
     return dict(beta=out[0], tv_before=out[1], tv_after=out[2], level=int(out[3]), steps=int(out[4]), accepted=int(out[5]))
+
+
+PCT_TVS_STATIC_MAX_SLOTS = 1 << 20
+
+
+def pct_tvs_step_static(image, nx, ny, nz, beta, n_halvings=4, info=None, cuda_stream=None):
+    """One TVS step on a caller-owned CUDA tensor without any device allocation (include/pct.h: pct_tvs_step_static).
+
+    For callers that cannot cudaMalloc while running (all device memory in their own pool, a latency-bound loop, a fixed
+    memory budget): the step's working memory is a fixed array inside the library.  image: float32 CUDA tensor of
+    nx*ny*nz values, overwritten; info: None or a float64 CUDA tensor of 4 (step used, TV before, TV after, level).
+    Calls that may overlap on the GPU share that array and race: keep them on one stream."""
+    rc = lib().pct_tvs_step_static(_ptr(image), int(nx), int(ny), int(nz), float(beta), int(n_halvings), _ptr(info), cuda_stream)
+    if rc != PCT_OK:
+        raise PctError(rc, lib().pct_tvs_step_static_error().decode())
 
 
 def pct_set_step(ctx, substeps):

@@ -109,7 +109,7 @@ class Histories:
         return s
 
     def hist(self, i):
-        p = int(self.proj[i])
+        p = min(int(self.proj[i]), int(self.proj_cos.shape[0]) - 1)  # DESIGN.md R24: clamped, as load_hist does in C
         return _Hist(*[float(self.a[k][i]) for k in _FIELDS[:8]], float(self.proj_cos[p]),
                      float(self.proj_sin[p]))
 

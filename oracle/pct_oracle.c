@@ -650,8 +650,10 @@ static void load_hist(const orc_histories *H, int64_t i, orc_hist *hh) {
     hh->t_in = H->t_in[i]; hh->v_in = H->v_in[i]; hh->t_out = H->t_out[i]; hh->v_out = H->v_out[i];
     hh->tht_in = H->tht_in[i]; hh->thv_in = H->thv_in[i];
     hh->tht_out = H->tht_out[i]; hh->thv_out = H->thv_out[i];
-    hh->cs = H->proj_cos[H->proj[i]];
-    hh->sn = H->proj_sin[H->proj[i]];
+    int p = H->proj[i];
+    if (p >= H->n_proj) p = H->n_proj - 1; /* DESIGN.md R24: an index past the tables means the last angle (never read out of bounds) */
+    hh->cs = H->proj_cos[p];
+    hh->sn = H->proj_sin[p];
 }
 
 /* Merged row of history i with fp64 lengths.  Returns nnz. */

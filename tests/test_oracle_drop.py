@@ -159,3 +159,35 @@ def test_p7_converges_to_dense_least_squares(oracle_mod, tiny):
     # and the error keeps shrinking monotonically sweep after sweep
     x2, _ = oracle_mod.drop_iterate(geom, hs, 1.9, 50, 200, x.copy())
     assert np.linalg.norm(x2[hit] - x_ls) < np.linalg.norm(x[hit] - x_ls)
+
+
+def test_r24_projection_index_past_the_tables_means_the_last_angle(oracle_mod):
+    """DESIGN.md R24 (the library's pct_set_histories promises it): proj[i] >= n_proj is read as n_proj - 1, never out of
+    bounds.  Pinned by substitution: histories whose index was pushed past the tables give, row by row and in a DROP
+    block, exactly what the same histories with the index written as n_proj - 1 give -- and NOT what angle 0 gives."""
+    geom, H = _tiny_problem(oracle_mod, n=600)
+    n_proj = H["proj_cos"].shape[0]
+    H["wepl"] = np.full(600, 5.0, dtype=np.float32)
+    bad = dict(H)
+    bad["proj"] = H["proj"].copy()
+    sel = np.arange(0, 600, 3)
+    bad["proj"][sel] = np.array([n_proj, n_proj + 5, 65535], dtype=np.uint16)[np.arange(sel.size) % 3]
+    want = dict(H)
+    want["proj"] = H["proj"].copy()
+    want["proj"][sel] = n_proj - 1
+    wrong = dict(H)
+    wrong["proj"] = H["proj"].copy()
+    wrong["proj"][sel] = 0
+    hb, hw, h0 = oracle_mod.Histories(bad), oracle_mod.Histories(want), oracle_mod.Histories(wrong)
+    differs = 0
+    for i in sel:
+        rb, rw, r0 = (oracle_mod.row_f32(geom, h.hist(int(i))) for h in (hb, hw, h0))
+        assert rb["nseg"] == rw["nseg"] and np.array_equal(rb["seg_idx"], rw["seg_idx"]) and np.array_equal(rb["seg_len"], rw["seg_len"])
+        differs += rb["nseg"] != r0["nseg"] or not np.array_equal(rb["seg_idx"], r0["seg_idx"])
+    assert differs > sel.size // 2  # the pin can tell the last angle from the first
+    x0 = np.linspace(0.5, 1.5, geom.n_voxels)
+    db, cb, _ = oracle_mod.block_accumulate(geom, hb, 0, 600, x0)   # the C loader (load_hist)
+    dw, cw, _ = oracle_mod.block_accumulate(geom, hw, 0, 600, x0)
+    d0, c0, _ = oracle_mod.block_accumulate(geom, h0, 0, 600, x0)
+    assert np.array_equal(db, dw) and np.array_equal(cb, cw)
+    assert not np.array_equal(cb, c0)

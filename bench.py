@@ -540,14 +540,17 @@ def run_carp_ranks(args):
         try:
             pct.pct_set_histories(ctx, hi - lo, D)
             _, n_slots = pct.pct_image_storage(ctx)
-            replicas.carp_distributed_pct(pct, ctx, cfg.n_voxels, cfg.lam, cfg.block_size, args.warmup, world, stream.cuda_stream)
+            tvs = args.tvs > 0  # one step per iteration on the common image, the placement of pct_iterate_carp
+            if tvs:
+                pct.pct_set_tvs(ctx, args.tvs, 1.0, 4)
+            replicas.carp_distributed_pct(pct, ctx, cfg.n_voxels, cfg.lam, cfg.block_size, args.warmup, world, stream.cuda_stream, tvs=tvs)
             pct.pct_synchronize(ctx)
             replicas.barrier(world)
             torch.cuda.synchronize()
             e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
             with ClockSampler(local) as clk:
                 e0.record()
-                replicas.carp_distributed_pct(pct, ctx, cfg.n_voxels, cfg.lam, cfg.block_size, args.steps, world, stream.cuda_stream)
+                replicas.carp_distributed_pct(pct, ctx, cfg.n_voxels, cfg.lam, cfg.block_size, args.steps, world, stream.cuda_stream, tvs=tvs)
                 e1.record()
                 torch.cuda.synchronize()
                 replicas.barrier(world)

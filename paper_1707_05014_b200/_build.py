@@ -8,7 +8,7 @@ _HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(_HERE, "csrc")
 LIB = os.path.join(_HERE, "libpct.so")
 _STAMP = LIB + ".stamp"
-SOURCES = ["pct_api.cu", "pct_kernels.cu", "pct_wave.cu", "pct_exact.cu", "pct_tvs.cu", "pct_peaks.cu", "pct_noalloc.cu"]
+SOURCES = ["pct_api.cu", "pct_kernels.cu", "pct_exact.cu", "pct_tvs.cu", "pct_peaks.cu", "pct_noalloc.cu"]
 HEADERS = ["pct_rule.cuh", "pct_walk.cuh", "pct_walk16.cuh", "pct_internal.h", os.path.join("..", "..", "include", "pct.h")]
 
 NVCC_FLAGS = [

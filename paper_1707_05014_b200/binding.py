@@ -10,8 +10,8 @@ import os
 
 from . import _build
 
-PCT_OK, PCT_EINVAL, PCT_ENOMEM, PCT_ECUDA, PCT_ESTATE = 0, -1, -2, -3, -4
-_STATUS = {0: "PCT_OK", -1: "PCT_EINVAL", -2: "PCT_ENOMEM", -3: "PCT_ECUDA", -4: "PCT_ESTATE"}
+PCT_OK, PCT_EINVAL, PCT_ENOMEM, PCT_ECUDA, PCT_ESTATE, PCT_EINTERNAL = 0, -1, -2, -3, -4, -5
+_STATUS = {0: "PCT_OK", -1: "PCT_EINVAL", -2: "PCT_ENOMEM", -3: "PCT_ECUDA", -4: "PCT_ESTATE", -5: "PCT_EINTERNAL"}
 
 FIELDS = ("entry_t", "entry_v", "exit_t", "exit_v", "entry_dt", "entry_dv", "exit_dt", "exit_dv", "wepl")
 
@@ -73,6 +73,8 @@ def lib():
         L.pct_set_tvs.argtypes = [vp, C.c_float, C.c_float, C.c_int]
         L.pct_set_step.argtypes = [vp, C.c_int]
         L.pct_set_walk.argtypes = [vp, C.c_int]
+        L.pct_set_option.argtypes = [vp, C.c_int, C.c_int]
+        L.pct_debug_rule_sweep.argtypes = [C.c_int, C.c_uint32, C.c_uint32, C.POINTER(C.c_uint64), vp]
         L.pct_image_storage.argtypes = [vp, C.POINTER(vp), C.POINTER(i64)]
         L.pct_tvs_step.argtypes = [vp]
         L.pct_get_tvs_state.argtypes = [vp, C.POINTER(C.c_double)]
@@ -85,7 +87,7 @@ def lib():
 EXPORTS = ("pct_create", "pct_set_histories", "pct_set_histories_host", "pct_set_histories_xyz", "pct_iterate", "pct_iterate_carp", "pct_set_path_model", "pct_get_image",
            "pct_set_image", "pct_synchronize", "pct_get_stats", "pct_destroy", "pct_last_error", "pct_version",
            "pct_debug_rows", "pct_debug_block", "pct_profile_sweep", "pct_measure_peaks", "pct_set_tvs", "pct_tvs_step", "pct_set_step", "pct_set_walk", "pct_image_storage",
-           "pct_get_tvs_state", "pct_tvs_step_static", "pct_tvs_step_static_error")
+           "pct_get_tvs_state", "pct_tvs_step_static", "pct_tvs_step_static_error", "pct_set_option", "pct_debug_rule_sweep")
 
 
 def _ptr(a):
@@ -194,6 +196,14 @@ def pct_debug_block(ctx, first, count, delta, cnt):
     _check(ctx, lib().pct_debug_block(ctx, int(first), int(count), _ptr(delta), _ptr(cnt)))
 
 
+def pct_debug_rule_sweep(which, first_bits, last_bits, cuda_stream=None):
+    """The rule's 1/a (which=0) or sqrt(a) (which=1) against the IEEE intrinsic on every fp32 bit pattern of the range
+    -> (number of mismatches, lowest mismatching pattern)."""
+    out = (C.c_uint64 * 2)()
+    _check(None, lib().pct_debug_rule_sweep(int(which), int(first_bits), int(last_bits), out, cuda_stream))
+    return int(out[0]), int(out[1])
+
+
 def pct_profile_sweep(ctx, lam, block_size):
     """One sweep with CUDA events around every launch -> dict of device times (include/pct.h)."""
     out = (C.c_float * 6)()
@@ -255,6 +265,12 @@ def pct_image_storage(ctx):
 
 
 PCT_WALK_MIDPOINT, PCT_WALK_EXACT = 0, 1
+PCT_OPT_ORDER, PCT_OPT_ROWS_PAIR = 0, 1
+
+
+def pct_set_option(ctx, key, value):
+    """PCT_OPT_ORDER 0/1/2 (depth-slab order inside a block: never / by footprint / always), PCT_OPT_ROWS_PAIR 0/1."""
+    _check(ctx, lib().pct_set_option(ctx, int(key), int(value)))
 
 
 def pct_set_walk(ctx, mode):

@@ -16,16 +16,6 @@
 
 using namespace pct;
 
-// Plan of the DROP blocks of one string of histories (the whole set for pct_iterate): where k_plan_blocks put its
-// results and how far it has got (blocks are planned as their histories arrive, include/pct.h pct_set_histories_host).
-struct WavePlan {
-    long long first = 0, n = 0;  // histories [first, first + n) of the context's set
-    long long n_blocks = 0, built = 0;
-    uint32_t* plan = nullptr;    // = plan_buf + first (borrowed)
-    int* need = nullptr;         // owned: [n_blocks][n_slabs]
-    int* done = nullptr;         // owned: [n_blocks][n_slabs]
-};
-
 struct pct_ctx {
     int device = 0;
     cudaStream_t stream = nullptr;
@@ -73,18 +63,9 @@ struct pct_ctx {
     float carp_graph_lambda = 0.f;
     long long carp_graph_block = 0, carp_graph_n = 0;
     const void *carp_graph_hist_key = nullptr, *carp_graph_order = nullptr, *carp_graph_scratch = nullptr;
-    // 0: the block engine (two launches per DROP block, replayed from a CUDA graph): the default, the faster one at
-    // every config measured; 1: the wavefront engine (pct_wave.cu, one persistent launch per sweep), PCT_ENGINE=wave
-    int engine = 0;
     int sm_count = 148;
-    int wave_grid = 0;
-    WaveShape shape{};
-    WaveCtrl* wctrl = nullptr;
-    uint32_t* plan_buf = nullptr;  // 4 B per history: processing order + slab range of every history (k_plan_blocks)
-    long long plan_block = 0;      // block size the plans were made for
-    int plan_strings = -1;         // 0: pct_iterate's blocks, P: the blocks of P CARP strings
-    std::vector<WavePlan> plans;   // one per string (one for DROP)
-    WaveCtrl* carp_wctrl = nullptr;
+    int opt_order = 1;  // pct_set_option(PCT_OPT_ORDER): depth-slab order of the histories inside a block -- 0 never, 1 by footprint, 2 always
+    bool opt_rows_pair = false;
     long long carp_stride = 0;     // voxels between the images / accumulators of two strings (a multiple of four)
     // exact-traversal walk (pct_set_walk): scratch of the lanes' runs, nullptr in the default (midpoint) mode
     float2* exact_scratch = nullptr;
@@ -191,10 +172,6 @@ static int wait_upload(pct_ctx* c, long long upto) {
     return PCT_OK;
 }
 
-#ifndef PCT_ORDER_BLOCKS
-#define PCT_ORDER_BLOCKS 1  // 0: never, 1: when image + accumulator exceed 85 % of the L2, 2: always
-#endif
-
 // The order buffer for this block size (4 B per history); without memory for it the blocks run in the
 // caller's order.  Slabs: image + accumulator (12 B per voxel) of one slab take a quarter of the L2, at
 // least 4 (measured at 256 x 256 x 160, 126 MB: 440 -> 317 us per 2e5-history block with 4 slabs, 318
@@ -207,9 +184,7 @@ static void prepare_order(pct_ctx* c, long long block_size, int strings = 0) {
     // ordering pays when image + accumulator do not fit the L2; for a grid that fits it is a wash (256 x 256 x
     // 128, 101 MB: sweep 906 -> 910 ms, and every upload would pay the sort), so such grids keep the caller's
     // order and its coalesced history loads
-    int mode = PCT_ORDER_BLOCKS;
-    if (const char* env = getenv("PCT_ORDER"))  // tuning / test override: 0 never, 1 by footprint, 2 always
-        if (env[0] >= '0' && env[0] <= '2' && env[1] == 0) mode = env[0] - '0';
+    const int mode = c->opt_order;  // pct_set_option(PCT_OPT_ORDER): 0 never, 1 by footprint (default), 2 always
     const bool wanted = mode == 2 || (mode == 1 && 12.0 * images * (double)c->n_slots > 0.85 * l2);
     if (!wanted || block_size < 1024) {  // (small blocks: nothing to gain)
         if (c->order) cudaFree(c->order);
@@ -238,21 +213,8 @@ static int build_order(pct_ctx* c, long long block_size, long long upto) {
     return PCT_OK;
 }
 
-static void release_plans(pct_ctx* c) {
-    for (WavePlan& pl : c->plans) {
-        if (pl.need) cudaFree(pl.need);
-        if (pl.done) cudaFree(pl.done);
-    }
-    c->plans.clear();
-    c->plan_block = 0;
-    c->plan_strings = -1;
-}
-
 static void release_histories(pct_ctx* c) {
     drop_graph(c);
-    release_plans(c);
-    if (c->plan_buf) cudaFree(c->plan_buf);
-    c->plan_buf = nullptr;
     if (c->order) cudaFree(c->order);
     c->order = nullptr;
     c->order_block = 0;
@@ -284,7 +246,11 @@ extern "C" int pct_create(pct_ctx** out, int nx, int ny, int nz, float h, float 
     if ((long long)nx * ny * nz >= (1LL << 31)) return fail(nullptr, PCT_EINVAL, "pct_create: nx*ny*nz must be < 2^31");
     if (!(h > 0.0f) || !isfinite(h)) return fail(nullptr, PCT_EINVAL, "pct_create: voxel_mm must be positive and finite");
     const int nmin = nx < ny ? nx : ny;
-    if (nmin > 2016) return fail(nullptr, PCT_EINVAL, "pct_create: min(nx,ny) must be <= 2016 (64 path segments per lane)");
+    if (((nmin + 32) >> 5) > 64 || drop_smem_bytes(nmin) + 1024 > (size_t)227 * 1024) {  // (1 KB: the kernels' static shared memory)
+        snprintf(g_create_err, 512, "pct_create: min(nx,ny) = %d is too wide: the rows of a CTA's warps and the staged tables need %zu B of "
+                 "shared memory, a B200 offers %d less 1 KB for the kernels' own (min(nx,ny) <= 1318)", nmin, drop_smem_bytes(nmin), 227 * 1024);
+        return PCT_EINVAL;
+    }
     // rule step G (fp32, this operation order)
     Geom g{};
     g.nx = nx; g.ny = ny; g.nz = nz; g.nmin = nmin;
@@ -335,20 +301,15 @@ extern "C" int pct_create(pct_ctx** out, int nx, int ny, int nz, float h, float 
         free(tab);
         CUDA_TRY(nullptr, e);
         CUDA_TRY(nullptr, cudaDeviceGetAttribute(&c->sm_count, cudaDevAttrMultiProcessorCount, c->device));
-        CUDA_TRY(nullptr, cudaMalloc(&c->wctrl, sizeof(WaveCtrl)));
-        CUDA_TRY(nullptr, cudaMemsetAsync(c->wctrl, 0, sizeof(WaveCtrl), c->stream));
-        c->shape = wave_shape(c->g);
-        if (const char* env = getenv("PCT_ENGINE")) c->engine = strcmp(env, "wave") == 0 ? 1 : 0;
         // the per-warp row buffer and the two staged copies of the table must fit the shared memory of an SM
         int smem_max = 0;
         CUDA_TRY(nullptr, cudaDeviceGetAttribute(&smem_max, cudaDevAttrMaxSharedMemoryPerBlockOptin, c->device));
-        if (wave_smem_need(nmin) > (size_t)smem_max) {
+        if (drop_smem_bytes(nmin) + 1024 > (size_t)smem_max) {
             snprintf(g_create_err, 512, "pct_create: min(nx,ny) = %d needs %zu B of shared memory per CTA, the device offers %d",
-                     nmin, wave_smem_need(nmin), smem_max);
+                     nmin, drop_smem_bytes(nmin), smem_max);
             return PCT_EINVAL;
         }
         CUDA_TRY(nullptr, drop_configure(nmin, &c->drop_grid));
-        CUDA_TRY(nullptr, wave_configure(nmin, &c->wave_grid));
         return PCT_OK;
     };
     rc = body();
@@ -379,8 +340,6 @@ static void release_carp(pct_ctx* c) {
     if (c->carp_x) cudaFree(c->carp_x);
     if (c->carp_acc) cudaFree(c->carp_acc);
     if (c->carp_ctrl) cudaFree(c->carp_ctrl);
-    if (c->carp_wctrl) cudaFree(c->carp_wctrl);
-    c->carp_wctrl = nullptr;
     c->carp_x = nullptr;
     c->carp_acc = nullptr;
     c->carp_ctrl = nullptr;
@@ -398,7 +357,6 @@ extern "C" void pct_destroy(pct_ctx* c) {
     if (c->acc) cudaFree(c->acc);
     if (c->tab) cudaFree(c->tab);
     if (c->ctrl) cudaFree(c->ctrl);
-    if (c->wctrl) cudaFree(c->wctrl);
     if (c->exact_scratch) cudaFree(c->exact_scratch);
     if (c->tvs_grad) cudaFree(c->tvs_grad);
     if (c->tvs_state) cudaFree(c->tvs_state);
@@ -526,7 +484,6 @@ static int set_histories_host_impl(pct_ctx* c, int64_t n, const pct_histories* h
         c->chunk_end.clear();
         c->chunks_waited = 0;
         c->order_built = 0;  // same buffer, new histories: the blocks are ordered again as they arrive
-        for (WavePlan& pl : c->plans) pl.built = 0;  // and planned again
         cudaEvent_t tail = nullptr;
         CUDA_TRY(c, cudaEventCreateWithFlags(&tail, cudaEventDisableTiming));
         cudaError_t e = cudaEventRecord(tail, c->stream);
@@ -613,147 +570,6 @@ static int capture_pairs(pct_ctx* c, const DropArgs& a, int grid, float lambda, 
 }
 
 
-// ---- wavefront engine: plans and sweeps (pct_wave.cu) ----------------------------------------------------------
-
-static HistPtrs offset_hist(HistPtrs H, long long lo) {
-    H.t_in += lo; H.v_in += lo; H.t_out += lo; H.v_out += lo;
-    H.dt_in += lo; H.dv_in += lo; H.dt_out += lo; H.dv_out += lo;
-    H.wepl += lo; H.proj += lo;
-    return H;
-}
-
-// The plans of the DROP blocks of `strings` strings (0: one plan over all histories; P: the P strings of CARP,
-// string p = histories [floor(p n / P), floor((p+1) n / P)), blocks counted from the string's first history, R27).
-static int ensure_plans(pct_ctx* c, long long block_size, int strings) {
-    if (!c->plans.empty() && c->plan_block == block_size && c->plan_strings == strings) return PCT_OK;
-    release_plans(c);
-    if (!c->plan_buf) CUDA_TRY(c, cudaMalloc(&c->plan_buf, sizeof(uint32_t) * (size_t)c->n));
-    const int P = strings > 0 ? strings : 1;
-    c->plans.resize(P);
-    for (int p = 0; p < P; ++p) {
-        WavePlan& pl = c->plans[p];
-        const long long lo = (long long)(((__int128)p * c->n) / P), hi = (long long)(((__int128)(p + 1) * c->n) / P);
-        pl.first = lo;
-        pl.n = hi - lo;
-        pl.n_blocks = (pl.n + block_size - 1) / block_size;
-        pl.built = 0;
-        pl.plan = c->plan_buf + lo;
-        const size_t cells = (size_t)pl.n_blocks * c->shape.n_slabs;
-        cudaError_t e = cudaMalloc(&pl.need, sizeof(int) * cells);
-        if (e == cudaSuccess) e = cudaMalloc(&pl.done, sizeof(int) * cells);
-        if (e != cudaSuccess) {
-            release_plans(c);
-            CUDA_TRY(c, e);
-        }
-    }
-    c->plan_block = block_size;
-    c->plan_strings = strings;
-    return PCT_OK;
-}
-
-// Plan blocks [built, upto) of the string (their histories must be on the device or on their way in stream order).
-static int build_plan(pct_ctx* c, WavePlan& pl, long long block_size, long long upto, cudaStream_t s) {
-    if (upto <= pl.built) return PCT_OK;
-    CUDA_TRY(c, launch_plan_blocks(offset_hist(c->H, pl.first), c->g, pl.n, block_size, pl.built, upto - pl.built, c->shape, pl.plan,
-                                   pl.need, s));
-    pl.built = upto;
-    return PCT_OK;
-}
-
-// Histories per work item: small enough that the items in flight (one per warp) cover well under a block, so that a
-// warp drawing the first item of block q+1 finds the first slabs of block q long updated (PCT_WAVE_ITEM overrides).
-static int wave_item(long long block_size, int grid) {
-    if (const char* env = getenv("PCT_WAVE_ITEM")) {
-        const int v = atoi(env);
-        if (v >= 1 && v <= 16) return v;
-    }
-    const long long warps = (long long)grid * wave_walkers_per_cta();
-    long long it = block_size / (2 * warps);
-    return it < 1 ? 1 : (it > 8 ? 8 : (int)it);
-}
-
-static WaveArgs wave_args(pct_ctx* c, const WavePlan* pl, long long block_size, float lambda, float* x, float2* acc, WaveCtrl* ctrl, int grid) {
-    WaveArgs a{};
-    a.g = c->g;
-    a.H = pl ? offset_hist(c->H, pl->first) : c->H;
-    a.n = pl ? pl->n : c->n;
-    a.block_size = block_size;
-    a.n_blocks = pl ? pl->n_blocks : 1;
-    a.item = wave_item(block_size, grid);
-    a.n_slabs = c->shape.n_slabs;
-    a.n_sub = c->shape.n_sub;
-    a.slab_voxels = (long long)c->shape.slab_slices * c->g.slice_p;
-    a.n_voxels = c->n_slots;
-    a.lambda = lambda;
-    a.x = x;
-    a.acc = acc;
-    a.tab = c->tab;
-    a.ctrl = ctrl;
-    a.plan = pl ? pl->plan : nullptr;
-    a.need = pl ? pl->need : nullptr;
-    a.done = pl ? pl->done : nullptr;
-    return a;
-}
-
-// One DROP sweep over the histories of a plan, image x, accumulator acc (zero on entry and on exit), on stream s.
-// on_main: s is the context's stream and the histories may still be uploading (the launches then follow the upload
-// 64 blocks at a time).  launches (optional) counts the k_wave launches.
-static int wave_sweep(pct_ctx* c, WavePlan& pl, long long block_size, float lambda, float* x, float2* acc, WaveCtrl* ctrl, int grid,
-                      cudaStream_t s, bool on_main, int* launches = nullptr) {
-    // the sweep's queue, flags and counters start from zero (`error` is sticky, `last` holds the previous sweep's counters)
-    CUDA_TRY(c, cudaMemsetAsync(ctrl, 0, offsetof(WaveCtrl, error), s));
-    CUDA_TRY(c, cudaMemsetAsync(ctrl->cur, 0, sizeof(ctrl->cur), s));
-    CUDA_TRY(c, cudaMemsetAsync(ctrl->upd_seq, 0, 5 * sizeof(ctrl->upd_seq), s));
-    CUDA_TRY(c, cudaMemsetAsync(pl.done, 0, sizeof(int) * (size_t)pl.n_blocks * c->shape.n_slabs, s));
-    WaveArgs a = wave_args(c, &pl, block_size, lambda, x, acc, ctrl, grid);
-    long long seg = pl.n_blocks;  // blocks per launch (PCT_WAVE_SEG: a tuning knob; 1 = a kernel boundary after every block)
-    if (const char* env = getenv("PCT_WAVE_SEG")) {
-        const long long v = atoll(env);
-        if (v >= 1) seg = v;
-    }
-    for (long long q = 0; q < pl.n_blocks;) {
-        long long q1 = q + seg < pl.n_blocks ? q + seg : pl.n_blocks;
-        if (on_main) {
-            if (c->chunks_waited < c->chunk_ev.size() && q + kGraphPairs < q1) q1 = q + kGraphPairs;
-            if (int rc = wait_upload(c, q1 < pl.n_blocks ? pl.first + q1 * block_size : -1)) return rc;
-        }
-        if (int rc = build_plan(c, pl, block_size, q1, s)) return rc;
-        if (q > 0) CUDA_TRY(c, cudaMemsetAsync(&ctrl->ticket, 0, sizeof(ctrl->ticket), s));
-        a.q0 = q;
-        a.q1 = q1;
-        CUDA_TRY(c, launch_wave(a, grid, s));
-        if (launches) ++*launches;
-        q = q1;
-    }
-    CUDA_TRY(c, cudaMemcpyAsync(ctrl->last, ctrl->cur, sizeof(ctrl->cur), cudaMemcpyDeviceToDevice, s));
-    return PCT_OK;
-}
-
-// A wait that timed out or a row outside its planned slab range (both "cannot happen": DESIGN.md) is reported once.
-static int check_wave_error(pct_ctx* c) {
-    if (c->engine != 1) return PCT_OK;
-    unsigned err = 0;
-    CUDA_TRY(c, cudaMemcpyAsync(&err, &c->wctrl->error, sizeof(err), cudaMemcpyDeviceToHost, c->stream));
-    CUDA_TRY(c, cudaStreamSynchronize(c->stream));
-    for (int p = 0; p < c->carp_p && c->carp_wctrl; ++p) {
-        unsigned e = 0;
-        CUDA_TRY(c, cudaMemcpy(&e, &c->carp_wctrl[p].error, sizeof(e), cudaMemcpyDeviceToHost));
-        if (e) CUDA_TRY(c, cudaMemset(&c->carp_wctrl[p].error, 0, sizeof(e)));
-        err |= e;
-    }
-    if (!err) return PCT_OK;
-    CUDA_TRY(c, cudaMemsetAsync(&c->wctrl->error, 0, sizeof(err), c->stream));
-    return fail(c, PCT_EINTERNAL, "wavefront engine: %s; the image is not valid",
-                (err & 1u) ? "a path left the depth-slab range planned for it" : "a slab wait timed out");
-}
-
-static int iterate_wave(pct_ctx* c, float lambda, long long block_size, int n_iter) {
-    if (int rc = ensure_plans(c, block_size, 0)) return rc;
-    for (int it = 0; it < n_iter; ++it)
-        if (int rc = wave_sweep(c, c->plans[0], block_size, lambda, c->x, c->acc, c->wctrl, c->wave_grid, c->stream, true)) return rc;
-    return PCT_OK;
-}
-
 extern "C" int pct_iterate(pct_ctx* c, float lambda, int64_t block_size, int n_iter) {
     if (!c) return PCT_EINVAL;
     if (!c->have_hist) return fail(c, PCT_ESTATE, "pct_iterate: no histories set");
@@ -763,7 +579,6 @@ extern "C" int pct_iterate(pct_ctx* c, float lambda, int64_t block_size, int n_i
     if (n_iter == 0) return PCT_OK;
     DeviceGuard guard(c->device);
     const bool tvs = c->tvs_beta0 > 0.0f;  // a step on the image that enters every block: launches go out one by one
-    if (c->engine == 1 && !tvs && !c->exact_scratch) return iterate_wave(c, lambda, block_size, n_iter);
     const long long n_blocks = (c->n + block_size - 1) / block_size;
     const long long pairs = n_blocks * (long long)n_iter;
     CUDA_TRY(c, cudaMemsetAsync(c->ctrl, 0, sizeof(Ctrl), c->stream));
@@ -828,8 +643,6 @@ extern "C" int pct_iterate_carp(pct_ctx* c, float lambda, int64_t block_size, in
         CUDA_TRY(c, cudaMalloc(&c->carp_x, sizeof(float) * (size_t)stride * P));
         CUDA_TRY(c, cudaMalloc(&c->carp_acc, sizeof(float2) * (size_t)stride * P));
         CUDA_TRY(c, cudaMalloc(&c->carp_ctrl, sizeof(Ctrl) * P));
-        CUDA_TRY(c, cudaMalloc(&c->carp_wctrl, sizeof(WaveCtrl) * P));
-        CUDA_TRY(c, cudaMemsetAsync(c->carp_wctrl, 0, sizeof(WaveCtrl) * P, c->stream));
         CUDA_TRY(c, cudaMemsetAsync(c->carp_acc, 0, sizeof(float2) * (size_t)stride * P, c->stream));
         CUDA_TRY(c, cudaEventCreateWithFlags(&c->carp_fork, cudaEventDisableTiming));
         for (int p = 0; p < P; ++p) {
@@ -842,13 +655,8 @@ extern "C" int pct_iterate_carp(pct_ctx* c, float lambda, int64_t block_size, in
         }
         c->carp_p = P;
     }
-    const bool wave = c->engine == 1 && !c->exact_scratch;
-    if (wave) {
-        if (int rc = ensure_plans(c, block_size, P)) return rc;
-    } else {
-        prepare_order(c, block_size, P);
-    }
-    if (!wave && c->order && c->order_built == 0) {  // every string's blocks, ordered by depth slab (k_order_blocks)
+    prepare_order(c, block_size, P);
+    if (c->order && c->order_built == 0) {  // every string's blocks, ordered by depth slab (k_order_blocks)
         for (int p = 0; p < P; ++p) {
             const long long lo = (long long)(((__int128)p * c->n) / P), hi = (long long)(((__int128)(p + 1) * c->n) / P);
             HistPtrs Hs = c->H;
@@ -884,15 +692,6 @@ extern "C" int pct_iterate_carp(pct_ctx* c, float lambda, int64_t block_size, in
             float* xs = c->carp_x + (size_t)p * stride;
             CUDA_TRY(c, cudaStreamWaitEvent(s, c->carp_fork, 0));
             CUDA_TRY(c, cudaMemcpyAsync(xs, c->x, sizeof(float) * M, cudaMemcpyDeviceToDevice, s));  // the common x0
-            if (wave) {
-                // every string gets its share of the CTA slots: P persistent launches side by side
-                const int grid_p = (c->wave_grid + P - 1) / P;
-                if (int rc = wave_sweep(c, c->plans[p], block_size, lambda, xs, c->carp_acc + (size_t)p * stride, c->carp_wctrl + p, grid_p, s, false))
-                    return rc;
-                CUDA_TRY(c, cudaEventRecord(c->carp_done[p], s));
-                CUDA_TRY(c, cudaStreamWaitEvent(c->stream, c->carp_done[p], 0));
-                continue;
-            }
             CUDA_TRY(c, cudaMemsetAsync(c->carp_ctrl + p, 0, sizeof(Ctrl), s));
             DropArgs a = drop_args(c, block_size, -1, 0);
             a.H.t_in += lo; a.H.v_in += lo; a.H.t_out += lo; a.H.v_out += lo;
@@ -923,10 +722,7 @@ extern "C" int pct_iterate_carp(pct_ctx* c, float lambda, int64_t block_size, in
         }
         CUDA_TRY(c, launch_mean(c->x, c->carp_x, P, M, stride, c->stream));
         // pct_get_stats: the counters of the strings' sweeps, added up
-        if (wave)
-            CUDA_TRY(c, launch_sum_stats(c->wctrl->last, c->carp_wctrl[0].last, sizeof(WaveCtrl), P, c->stream));
-        else
-            CUDA_TRY(c, launch_sum_stats(c->ctrl->last, c->carp_ctrl[0].last, sizeof(Ctrl), P, c->stream));
+        CUDA_TRY(c, launch_sum_stats(c->ctrl->last, c->carp_ctrl[0].last, sizeof(Ctrl), P, c->stream));
     }
     return PCT_OK;
 }
@@ -997,8 +793,11 @@ extern "C" int pct_set_step(pct_ctx* c, int substeps) {
     if (kmax == c->g.kmax) return PCT_OK;
     int smem_max = 0;
     CUDA_TRY(c, cudaDeviceGetAttribute(&smem_max, cudaDevAttrMaxSharedMemoryPerBlockOptin, c->device));
-    if (((kmax + 32) >> 5) > 64 || wave_smem_need(kmax) > (size_t)smem_max)
-        return fail(c, PCT_EINVAL, "pct_set_step: the grid is too wide for the half-voxel step (row buffer does not fit shared memory)");
+    if (((kmax + 32) >> 5) > 64 || drop_smem_bytes(kmax) + 1024 > (size_t)smem_max) {
+        char what[96];
+        snprintf(what, sizeof(what), "%zu B of shared memory per CTA needed, %d offered", drop_smem_bytes(kmax), smem_max);
+        return fail(c, PCT_EINVAL, "pct_set_step: the grid is too wide for the half-voxel step (%s)", what);
+    }
     const float step = substeps == 2 ? 0.5f * c->g.h : c->g.h;
     float4* tab = (float4*)malloc(sizeof(float4) * (kmax + 1));
     if (!tab) return fail(c, PCT_ENOMEM, "pct_set_step: out of host memory");
@@ -1008,7 +807,6 @@ extern "C" int pct_set_step(pct_ctx* c, int substeps) {
     free(tab);
     CUDA_TRY(c, e);
     CUDA_TRY(c, drop_configure(kmax, &c->drop_grid));
-    CUDA_TRY(c, wave_configure(kmax, &c->wave_grid));
     c->g.kmax = kmax;
     c->g.inv_step = 1.0f / step;
     drop_graph(c);  // the cached graph holds the old geometry
@@ -1040,6 +838,22 @@ extern "C" int pct_set_walk(pct_ctx* c, int mode) {
     return exact_scratch_alloc(c);
 }
 
+extern "C" int pct_set_option(pct_ctx* c, int key, int value) {
+    if (!c) return PCT_EINVAL;
+    switch (key) {
+        case PCT_OPT_ORDER:
+            if (value < 0 || value > 2) return fail(c, PCT_EINVAL, "pct_set_option: PCT_OPT_ORDER takes 0 (never), 1 (by footprint) or 2 (always)");
+            c->opt_order = value;  // takes effect at the next pct_iterate / pct_iterate_carp (prepare_order)
+            return PCT_OK;
+        case PCT_OPT_ROWS_PAIR:
+            if (value != 0 && value != 1) return fail(c, PCT_EINVAL, "pct_set_option: PCT_OPT_ROWS_PAIR takes 0 or 1");
+            c->opt_rows_pair = value == 1;
+            return PCT_OK;
+        default:
+            return fail(c, PCT_EINVAL, "pct_set_option: unknown key");
+    }
+}
+
 extern "C" int pct_set_path_model(pct_ctx* c, int model) {
     if (!c) return PCT_EINVAL;
     if (model != PCT_PATH_MLP && model != PCT_PATH_SPLINE) return fail(c, PCT_EINVAL, "pct_set_path_model: unknown model");
@@ -1050,12 +864,23 @@ extern "C" int pct_set_path_model(pct_ctx* c, int model) {
     return PCT_OK;
 }
 
+// Exact traversal: a history whose runs outgrow its lane's scratch is left out of its block and counted (pct_exact.cu);
+// the count of the last sweep is in ctrl->last[3].  Called after the stream has been synchronised.
+static const char kExactOverflow[] = "exact traversal: a path produced more runs than a lane's scratch holds (slopes beyond any tracker's); its row was left out";
+static int check_exact_error(pct_ctx* c) {
+    if (!c->exact_scratch) return PCT_OK;
+    unsigned long long dropped = 0;
+    CUDA_TRY(c, cudaMemcpyAsync(&dropped, &c->ctrl->last[3], sizeof(dropped), cudaMemcpyDeviceToHost, c->stream));
+    CUDA_TRY(c, cudaStreamSynchronize(c->stream));
+    return dropped ? fail(c, PCT_EINTERNAL, "%s", kExactOverflow) : PCT_OK;
+}
+
 extern "C" int pct_synchronize(pct_ctx* c) {
     if (!c) return PCT_EINVAL;
     DeviceGuard guard(c->device);
     if (int rc = wait_upload(c, -1)) return rc;  // the host arrays are free once this returns
     CUDA_TRY(c, cudaStreamSynchronize(c->stream));
-    return check_wave_error(c);
+    return check_exact_error(c);
 }
 
 extern "C" int pct_get_image(pct_ctx* c, float* dst, int64_t n_voxels) {
@@ -1068,7 +893,7 @@ extern "C" int pct_get_image(pct_ctx* c, float* dst, int64_t n_voxels) {
     CUDA_TRY(c, launch_image_io(c->x, out, c->g, false, c->stream));
     if (out != dst) CUDA_TRY(c, cudaMemcpyAsync(dst, out, sizeof(float) * c->n_voxels, cudaMemcpyDeviceToHost, c->stream));
     CUDA_TRY(c, cudaStreamSynchronize(c->stream));
-    return check_wave_error(c);
+    return check_exact_error(c);
 }
 
 extern "C" int pct_set_image(pct_ctx* c, const float* src, int64_t n_voxels) {
@@ -1093,16 +918,14 @@ extern "C" int pct_get_stats(pct_ctx* c, int64_t out[4]) {
     if (!c || !out) return PCT_EINVAL;
     DeviceGuard guard(c->device);
     unsigned long long last[4] = {0, 0, 0, 0};
-    const void* src = (c->engine == 1 && !c->exact_scratch) ? (const void*)c->wctrl->last : (const void*)c->ctrl->last;
-    CUDA_TRY(c, cudaMemcpyAsync(last, src, sizeof(last), cudaMemcpyDeviceToHost, c->stream));
+    CUDA_TRY(c, cudaMemcpyAsync(last, c->ctrl->last, sizeof(last), cudaMemcpyDeviceToHost, c->stream));
     CUDA_TRY(c, cudaStreamSynchronize(c->stream));
     for (int i = 0; i < 3; ++i) out[i] = (int64_t)last[i];
     out[3] = c->n;
     if (c->exact_scratch && last[3] > 0)
-        return fail(c, PCT_EINTERNAL, "exact traversal: a path produced more runs than a lane's scratch holds (slopes beyond any tracker's)");
-    wave_prof_dump("pct_get_stats");
+        return fail(c, PCT_EINTERNAL, "%s", kExactOverflow);
     bounds_dump("pct_get_stats");
-    return check_wave_error(c);
+    return PCT_OK;
 }
 
 extern "C" int pct_debug_rows(pct_ctx* c, int64_t first, int64_t count, int32_t max_seg, int32_t* nseg, int32_t* nnz,
@@ -1130,7 +953,7 @@ extern "C" int pct_debug_rows(pct_ctx* c, int64_t first, int64_t count, int32_t 
         CUDA_TRY(c, launch_rows_exact(a, c->sm_count, c->stream));
         return PCT_OK;
     }
-    CUDA_TRY(c, launch_rows(a, c->stream));
+    CUDA_TRY(c, launch_rows(a, c->opt_rows_pair, c->stream));
     return PCT_OK;
 }
 
@@ -1143,21 +966,29 @@ extern "C" int pct_debug_block(pct_ctx* c, int64_t first, int64_t count, float* 
     if (count > (1LL << 24)) return fail(c, PCT_EINVAL, "pct_debug_block: count must be <= 2^24 (hit counts are held exactly in fp32)");
     DeviceGuard guard(c->device);
     if (int rc = wait_upload(c, first + count)) return rc;
-    if (c->engine == 1 && !c->exact_scratch) {  // the wavefront kernel in its plain mode: the range as ONE block in the caller's order, no update
-        CUDA_TRY(c, cudaMemsetAsync(&c->wctrl->ticket, 0, sizeof(c->wctrl->ticket), c->stream));
-        WaveArgs w = wave_args(c, nullptr, count, 1.0f, c->x, c->acc, c->wctrl, c->wave_grid);
-        w.first = first;
-        w.count = count;
-        CUDA_TRY(c, launch_wave(w, c->wave_grid, c->stream));
-        CUDA_TRY(c, launch_split_acc(c->acc, delta, cnt, c->g, c->stream));
-        CUDA_TRY(c, cudaMemsetAsync(c->wctrl->cur, 0, sizeof(c->wctrl->cur), c->stream));
-        return PCT_OK;
-    }
     CUDA_TRY(c, cudaMemsetAsync(c->ctrl, 0, sizeof(Ctrl), c->stream));
     const DropArgs a = drop_args(c, count, first, count);
     CUDA_TRY(c, launch_drop_block(a, c->drop_grid, c->stream));
     CUDA_TRY(c, launch_split_acc(c->acc, delta, cnt, c->g, c->stream));
     CUDA_TRY(c, cudaMemsetAsync(c->ctrl, 0, sizeof(Ctrl), c->stream));
+    return PCT_OK;
+}
+
+extern "C" int pct_debug_rule_sweep(int which, uint32_t first_bits, uint32_t last_bits, uint64_t out[2], void* cuda_stream) {
+    if (!out || (which != 0 && which != 1) || first_bits > last_bits) return fail(nullptr, PCT_EINVAL, "pct_debug_rule_sweep: which must be 0 or 1, first_bits <= last_bits, out not NULL");
+    unsigned long long* d = nullptr;
+    const unsigned long long init[2] = {0ULL, ~0ULL};
+    unsigned long long res[2] = {0ULL, 0ULL};
+    cudaStream_t s = (cudaStream_t)cuda_stream;
+    CUDA_TRY(nullptr, cudaMalloc(&d, sizeof(init)));
+    cudaError_t e = cudaMemcpyAsync(d, init, sizeof(init), cudaMemcpyHostToDevice, s);
+    if (e == cudaSuccess) e = launch_rule_sweep(which, first_bits, last_bits, d, s);
+    if (e == cudaSuccess) e = cudaMemcpyAsync(res, d, sizeof(res), cudaMemcpyDeviceToHost, s);
+    if (e == cudaSuccess) e = cudaStreamSynchronize(s);
+    cudaFree(d);
+    CUDA_TRY(nullptr, e);
+    out[0] = res[0];
+    out[1] = res[0] ? res[1] : 0ULL;
     return PCT_OK;
 }
 
@@ -1170,30 +1001,6 @@ extern "C" int pct_profile_sweep(pct_ctx* c, float lambda, int64_t block_size, f
     DeviceGuard guard(c->device);
     if (int rc = wait_upload(c, -1)) return rc;
     const long long n_blocks = (c->n + block_size - 1) / block_size;
-    if (c->engine == 1 && !c->exact_scratch) {  // one persistent launch per sweep: its device time IS the sweep's
-        if (int rc = ensure_plans(c, block_size, 0)) return rc;
-        if (int rc = build_plan(c, c->plans[0], block_size, n_blocks, c->stream)) return rc;  // (the plan is made once per history set: not timed)
-        cudaEvent_t e0 = nullptr, e1 = nullptr;
-        CUDA_TRY(c, cudaEventCreate(&e0));
-        cudaError_t e = cudaEventCreate(&e1);
-        int launches = 0, rc = PCT_OK;
-        float ms = 0.f;
-        if (e == cudaSuccess) e = cudaEventRecord(e0, c->stream);
-        if (e == cudaSuccess) rc = wave_sweep(c, c->plans[0], block_size, lambda, c->x, c->acc, c->wctrl, c->wave_grid, c->stream, true, &launches);
-        if (e == cudaSuccess && rc == PCT_OK) e = cudaEventRecord(e1, c->stream);
-        if (e == cudaSuccess && rc == PCT_OK) e = cudaStreamSynchronize(c->stream);
-        if (e == cudaSuccess && rc == PCT_OK) e = cudaEventElapsedTime(&ms, e0, e1);
-        cudaEventDestroy(e0);
-        if (e1) cudaEventDestroy(e1);
-        if (rc != PCT_OK) return rc;
-        CUDA_TRY(c, e);
-        out_ms[0] = ms;
-        out_ms[1] = 0.f;
-        out_ms[2] = ms;
-        out_ms[3] = (float)launches;
-        out_ms[4] = out_ms[5] = 0.f;
-        return check_wave_error(c);
-    }
     const int kChunk = 256;  // blocks per batch of events
     cudaEvent_t ev[3 * kChunk + 1];  // per block: [TVS step] accumulate, update
     int made = 0;

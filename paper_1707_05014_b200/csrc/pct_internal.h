@@ -70,69 +70,13 @@ cudaError_t launch_xyz_to_beam(float u_pl, long long n, const float* x, const fl
                                const uint16_t* proj, const float* pcos, const float* psin, int n_proj, float* t_out, float* v_out,
                                cudaStream_t stream);
 cudaError_t launch_image_io(float* x, float* ext, const Geom& g, bool to_storage, cudaStream_t stream);
-cudaError_t launch_rows(const RowsArgs& a, cudaStream_t stream);
+cudaError_t launch_rows(const RowsArgs& a, bool pair_walk, cudaStream_t stream);
+bool pair_enabled(int kmax);  // the two-histories-per-warp kernel serves this node count
+cudaError_t launch_sum_stats(unsigned long long* dst, const unsigned long long* src, size_t pitch, int n_strings, cudaStream_t stream);
+cudaError_t launch_rule_sweep(int which, uint32_t lo, uint32_t hi, unsigned long long* out, cudaStream_t stream);
 cudaError_t launch_mean(float* x, const float* xs, int n_strings, long long n_voxels, long long pitch, cudaStream_t stream);
 cudaError_t launch_order_blocks(const HistPtrs& H, const Geom& g, long long n, long long block_size, long long first_block,
                                 long long n_blocks, int n_slabs, uint32_t* order, cudaStream_t stream);
-
-// ---- wavefront engine (pct_wave.cu) -------------------------------------------------------------------------
-// A DROP block ends in a barrier only per DEPTH SLAB: a proton stays within a few slices of the image (mrad
-// slopes), so the histories of a block are planned by the slab range [sa, sb] their path can touch
-// (k_plan_blocks), the slab s of block q is updated as soon as every history of block q whose range holds s has
-// scattered, and a history of block q+1 waits only for the slabs of its own range.  One persistent launch runs a
-// whole range of blocks; what PAPER.md:50 prescribes -- every row of block q+1 sees the image after block q on
-// every voxel it touches -- holds exactly.
-constexpr int kMaxSlabs = 32;
-
-struct alignas(128) WaveCtrl {
-    unsigned long long ticket;    // next work item of the launch
-    unsigned int unused;
-    unsigned int error;           // sticky: 1 = a row left the slab range its plan declared, 2 = a wait timed out
-    unsigned long long cur[4];    // running counters of the current sweep: rows, nnz, segments, -
-    unsigned long long last[4];   // counters of the last completed sweep
-    unsigned int pad[12];
-    // indexed by slab, one or two 128 B lines each
-    unsigned int upd_seq[kMaxSlabs];   // the slab holds the image after blocks [0, upd_seq) of the sweep
-    unsigned int post_seq[kMaxSlabs];  // block whose update was posted last
-    unsigned int finished[kMaxSlabs];  // update sub-tasks finished so far (sweep)
-    unsigned long long tasks[kMaxSlabs];  // low half: update sub-tasks posted so far (sweep), high half: claimed so far
-};
-static_assert(sizeof(WaveCtrl) == 128 * 6, "WaveCtrl layout");
-
-struct WaveArgs {
-    Geom g;
-    HistPtrs H;
-    long long n;           // histories
-    long long block_size;  // DROP block size
-    long long n_blocks;
-    long long q0, q1;      // DROP blocks [q0, q1) of the sweep (planned mode)
-    long long first, count;  // plain mode (plan == nullptr): histories [first, first+count) as one block, no update
-    int item;              // histories per work item
-    int n_slabs, n_sub;
-    long long slab_voxels;  // voxels per slab (slices per slab * nx * ny): slab s = linear indices [s, s+1) * slab_voxels
-    long long n_voxels;
-    float lambda;
-    float* x;
-    float2* acc;
-    const float4* tab;
-    WaveCtrl* ctrl;
-    const uint32_t* plan;  // per position of the block's processing order: offset in the block | sa << 24 | width code << 29
-    const int* need;       // [n_blocks][n_slabs] histories of the block whose slab range holds the slab
-    int* done;             // [n_blocks][n_slabs] of them, how many have scattered (zeroed per sweep)
-};
-
-struct WaveShape {
-    int n_slabs, slab_slices, n_sub;
-};
-WaveShape wave_shape(const Geom& g);
-int wave_walkers_per_cta();
-size_t wave_smem_need(int nmin);
-cudaError_t wave_configure(int nmin, int* grid_out);
-void wave_prof_dump(const char* tag);  // (a no-op unless built with -DPCT_WAVE_PROF)
-cudaError_t launch_sum_stats(unsigned long long* dst, const unsigned long long* src, size_t pitch, int n_strings, cudaStream_t stream);
-cudaError_t launch_wave(const WaveArgs& a, int grid, cudaStream_t stream);
-cudaError_t launch_plan_blocks(const HistPtrs& H, const Geom& g, long long n, long long block_size, long long first_block,
-                               long long n_blocks, const WaveShape& shp, uint32_t* plan, int* need, cudaStream_t stream);
 
 // ---- total-variation superiorization (pct_tvs.cu) ---------------------------------------------------------------
 constexpr int kTvMaxLevels = 8;

@@ -324,17 +324,13 @@ __global__ void __launch_bounds__(kThreads, kCtasPerSm) k_drop_pair(const DropAr
     }
 }
 
-// PCT_PAIR=0 selects the one-history-per-warp kernel (k_drop_block) everywhere.  The pair kernel is used where two of its
-// CTAs fit the shared memory of an SM like k_drop_block's do (not with the half-voxel step on wide grids: two row buffers
-// per warp of twice the length).
-static bool pair_enabled(int kmax) {
-    static int on = -1;
-    if (on < 0) {
-        const char* env = getenv("PCT_PAIR");
-        on = (env && env[0] == '0') ? 0 : 1;
-    }
-    return on == 1 && 2 * (drop_pair_smem_bytes(kmax) + 1024) <= 227 * 1024;
-}
+// The pair kernel is used where two of its CTAs fit the shared memory of an SM like k_drop_block's do (not with the
+// half-voxel step on wide grids, nor on grids wider than about 420 voxels: two row buffers per warp).  Building with
+// -DPCT_PAIR=0 selects the one-history-per-warp kernel (k_drop_block) everywhere (the A/B build of DESIGN.md).
+#ifndef PCT_PAIR
+#define PCT_PAIR 1
+#endif
+bool pair_enabled(int kmax) { return PCT_PAIR == 1 && 2 * (drop_pair_smem_bytes(kmax) + 1024) <= 227 * 1024; }
 
 cudaError_t drop_configure(int nmin, int* grid_out) {
     if (((nmin + 32) >> 5) > 64) return cudaErrorInvalidValue;
@@ -345,12 +341,15 @@ cudaError_t drop_configure(int nmin, int* grid_out) {
     if ((e = cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev)) != cudaSuccess) return e;
     e = cudaFuncSetAttribute(k_drop_block<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (e == cudaSuccess) e = cudaFuncSetAttribute(k_drop_block<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    // the pair kernel's two row buffers per warp outgrow the 227 KB opt-in limit on wide grids (kmax above about 850): it is
+    // configured, and its occupancy taken, only where it will run; elsewhere k_drop_block alone serves
     const size_t smem2 = drop_pair_smem_bytes(nmin);
-    if (e == cudaSuccess) e = cudaFuncSetAttribute(k_drop_pair<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem2);
-    if (e == cudaSuccess) e = cudaFuncSetAttribute(k_drop_pair<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem2);
+    const bool pair = pair_enabled(nmin);
+    if (pair && e == cudaSuccess) e = cudaFuncSetAttribute(k_drop_pair<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem2);
+    if (pair && e == cudaSuccess) e = cudaFuncSetAttribute(k_drop_pair<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem2);
     if (e == cudaSuccess)
-        e = pair_enabled(nmin) ? cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, k_drop_pair<false>, kThreads, smem2)
-                           : cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, k_drop_block<false>, kThreads, smem);
+        e = pair ? cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, k_drop_pair<false>, kThreads, smem2)
+                 : cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, k_drop_block<false>, kThreads, smem);
     if (e != cudaSuccess) return e;
     if (per_sm < 1) return cudaErrorLaunchOutOfResources;
     *grid_out = sms * per_sm;  // persistent: every CTA slot of the chip, work handed out dynamically
@@ -359,15 +358,10 @@ cudaError_t drop_configure(int nmin, int* grid_out) {
 
 // Launch with the programmatic-stream-serialization attribute: the grid may be scheduled as soon as the previous
 // kernel in the stream lets its SM slots go; the kernel itself waits (griddepcontrol.wait) before it reads anything
-// the previous kernel writes.  PCT_PDL=0 launches the plain way.
-static bool pdl_enabled() {
-    static int on = -1;
-    if (on < 0) {
-        const char* env = getenv("PCT_PDL");
-        on = (env && env[0] == '0') ? 0 : 1;
-    }
-    return on == 1;
-}
+// the previous kernel writes.  A build with -DPCT_PDL=0 launches the plain way.
+#ifndef PCT_PDL
+#define PCT_PDL 1
+#endif
 
 template <typename... KArgs, typename... Args>
 static cudaError_t launch_pdl(void (*kernel)(KArgs...), dim3 grid, dim3 block, size_t smem, cudaStream_t stream, Args... args) {
@@ -380,7 +374,7 @@ static cudaError_t launch_pdl(void (*kernel)(KArgs...), dim3 grid, dim3 block, s
     attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
     attr[0].val.programmaticStreamSerializationAllowed = 1;
     cfg.attrs = attr;
-    cfg.numAttrs = pdl_enabled() ? 1 : 0;
+    cfg.numAttrs = PCT_PDL ? 1 : 0;
     return cudaLaunchKernelEx(&cfg, kernel, args...);
 }
 
@@ -636,7 +630,7 @@ __global__ void __launch_bounds__(kThreads) k_rows(const RowsArgs a) {
     }
 }
 
-// inspection of the two-histories-per-warp walk (pct_walk16.cuh; PCT_ROWS_PAIR=1): histories (2 w, 2 w + 1) of the range
+// inspection of the two-histories-per-warp walk (pct_walk16.cuh; pct_set_option PCT_OPT_ROWS_PAIR): histories (2 w, 2 w + 1) of the range
 // are walked side by side exactly as k_drop_pair walks a pair, and the rows are read back from the two row buffers.
 // Node positions are not written by this walk (they are k_rows's, the same node_pair code).
 template <bool SPLINE>
@@ -715,7 +709,7 @@ __global__ void __launch_bounds__(kThreads) k_rows_pair(const RowsArgs a) {
     }
 }
 
-cudaError_t launch_rows(const RowsArgs& a, cudaStream_t stream) {
+cudaError_t launch_rows(const RowsArgs& a, bool pair_walk, cudaStream_t stream) {
     if (((a.g.kmax + 32) >> 5) > 64) return cudaErrorInvalidValue;
     const size_t smem = drop_smem_bytes(a.g.kmax);
     long long blocks = (a.count + kWarpsPerCta - 1) / kWarpsPerCta;
@@ -723,8 +717,7 @@ cudaError_t launch_rows(const RowsArgs& a, cudaStream_t stream) {
     if (blocks > cap) blocks = cap;
     if (blocks < 1) blocks = 1;
     cudaError_t e = cudaSuccess;
-    const char* env = getenv("PCT_ROWS_PAIR");
-    if (env && env[0] == '1' && a.nodes == nullptr && pair_enabled(a.g.kmax)) {  // the hot path's pair walk, inspected
+    if (pair_walk && a.nodes == nullptr && pair_enabled(a.g.kmax)) {  // the hot path's pair walk, inspected
         const size_t smem2 = drop_pair_smem_bytes(a.g.kmax);
         if (a.g.path_model == 1) {
             e = cudaFuncSetAttribute(k_rows_pair<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem2);
@@ -863,6 +856,34 @@ cudaError_t launch_mean(float* x, const float* xs, int n_strings, long long n, l
 
 // pct_get_stats after CARP: the counters of the strings' last sweeps, added up into the context's.  src = the `last`
 // array of string 0, the strings' control blocks `pitch` bytes apart.
+// inspection: the rule's 1/a and sqrt(a) (pct_rule.cuh: hardware approximation + one FMA Newton step, no range test)
+// against the IEEE intrinsics __frcp_rn / __fsqrt_rn for EVERY fp32 bit pattern in [lo, hi] -- the argument ranges the
+// rule feeds them are swept in full by tests/test_gpu_parity.py.  out[0] counts the patterns whose results
+// differ in any bit, out[1] keeps the lowest such pattern.
+__global__ void k_rule_sweep(int which, uint32_t lo, uint32_t hi, unsigned long long* out) {
+    const unsigned long long n = (unsigned long long)hi - lo + 1ULL, pairs = (n + 1ULL) >> 1;
+    const unsigned long long stride = (unsigned long long)gridDim.x * blockDim.x;
+    unsigned long long bad = 0ULL, first = ~0ULL;
+    for (unsigned long long q = (unsigned long long)blockIdx.x * blockDim.x + threadIdx.x; q < pairs; q += stride) {
+        const unsigned long long b0 = lo + 2ULL * q, b1 = b0 + 1ULL <= hi ? b0 + 1ULL : b0;
+        const float a0 = __uint_as_float((uint32_t)b0), a1 = __uint_as_float((uint32_t)b1);
+        float r0, r1;
+        upk(which == 0 ? rcp_rn_normal2(pk(a0, a1)) : sqrt_rn_normal2(pk(a0, a1)), r0, r1);
+        const float w0 = which == 0 ? __frcp_rn(a0) : __fsqrt_rn(a0), w1 = which == 0 ? __frcp_rn(a1) : __fsqrt_rn(a1);
+        if (__float_as_uint(r0) != __float_as_uint(w0)) ++bad, first = b0 < first ? b0 : first;
+        if (b1 != b0 && __float_as_uint(r1) != __float_as_uint(w1)) ++bad, first = b1 < first ? b1 : first;
+    }
+    if (bad) {
+        atomicAdd(&out[0], bad);
+        atomicMin(&out[1], first);
+    }
+}
+
+cudaError_t launch_rule_sweep(int which, uint32_t lo, uint32_t hi, unsigned long long* out, cudaStream_t stream) {
+    k_rule_sweep<<<sm_count() * 8, 256, 0, stream>>>(which, lo, hi, out);
+    return cudaGetLastError();
+}
+
 __global__ void k_sum_stats(unsigned long long* dst, const unsigned long long* src, size_t pitch, int n_strings) {
     if (threadIdx.x < 4) {
         unsigned long long s = 0;

@@ -1,5 +1,5 @@
 // pct_walk.cuh -- device functions shared by the kernels of the hot path (pct_kernels.cu: the block engine and the
-// inspection kernels; pct_wave.cu: the wavefront engine): Sigma1^-1 table staging, history loads, the per-warp row
+// inspection kernels): Sigma1^-1 table staging, history loads, the per-warp row
 // buffer, the lane-chunked walk of one history by one warp (rule steps 3-4) and the segment-major
 // gather (a_i.x) and scatter ((Delta_j, c_j) += ...) passes (R12).
 #pragma once
@@ -398,42 +398,6 @@ __device__ __forceinline__ void scatter_row(const float2* row, int lane, int C, 
 #define PCT_S(N) scatter_n<N>(rl + 33 * i, acc, r)
     PCT_SWITCH_N(C - i, PCT_S);
 #undef PCT_S
-}
-
-// ---- the same gather for the wavefront engine (pct_wave.cu) -----------------------------------------------
-// The image is UPDATED by other SMs while the kernel runs (slab by slab, ordered by flags), so it is read with
-// ld.global.cg (L2 only: the L1 is not coherent and could hold a line from before an update).  `bad` collects
-// whether a voxel of the row lies outside [lo, lo + span): the slab range the block plan declared for the history.
-template <int N>
-__device__ __forceinline__ float gather_cg_n(const float2* rl, const float* x, unsigned lo, unsigned span, bool& bad) {
-    float2 e[N];
-    float xv[N];
-#pragma unroll
-    for (int u = 0; u < N; ++u) e[u] = rl[33 * u];
-#pragma unroll
-    for (int u = 0; u < N; ++u) {
-        const int lin = __float_as_int(e[u].x);
-        xv[u] = 0.0f;
-        if (lin >= 0) {
-            xv[u] = __ldcg(x + lin);
-            bad |= (unsigned)lin - lo >= span;
-        }
-    }
-    float dot = 0.0f;
-#pragma unroll
-    for (int u = 0; u < N; ++u) dot = __fmaf_rn(fabsf(e[u].y), xv[u], dot);
-    return dot;
-}
-
-__device__ __forceinline__ float gather_row_cg(const float2* row, int lane, int C, const float* x, unsigned lo, unsigned span, bool& bad) {
-    const float2* rl = row + lane;
-    float dot = 0.0f;
-    int i = 0;
-    for (; i + 8 <= C; i += 8) dot += gather_cg_n<8>(rl + 33 * i, x, lo, span, bad);
-#define PCT_G(N) dot += gather_cg_n<N>(rl + 33 * i, x, lo, span, bad)
-    PCT_SWITCH_N(C - i, PCT_G);
-#undef PCT_G
-    return dot;
 }
 
 }  // namespace pct

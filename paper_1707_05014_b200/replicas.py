@@ -74,16 +74,29 @@ class _DeviceArray:
         self.__cuda_array_interface__ = {"shape": (int(n),), "typestr": "<f4", "data": (int(address), False), "version": 3}
 
 
-def carp_distributed_pct(pct, ctx, n_voxels, lam, block_size, n_iter, world, ctx_stream=None):
+def carp_distributed_pct(pct, ctx, n_voxels, lam, block_size, n_iter, world, ctx_stream=None, tvs=False):
     """carp_distributed on a libpct context holding this rank's string (pct = the binding module).
 
     The average is taken IN PLACE on the library's own image array (pct_image_storage: the storage order is the same
     on every rank of the same grid, and a sum does not care about order): no copy, no host synchronisation.  All of it
     is ordered on the context's stream: ctx_stream is the cudaStream_t handle given to pct_create (None: the context was
     created on torch's current stream), and the collective and the division run under that stream, so the sweep, the
-    all-reduce and the next sweep follow one another on the device."""
+    all-reduce and the next sweep follow one another on the device.
+
+    TVS (pct_set_tvs).  PAPER.md:113: "In CARP, TVS is applied just once to the initial solution at the start of each
+    iteration" -- not before every block, which is where pct_iterate puts it (the DROP placement).  With tvs=True the
+    rank's sweep is pct_iterate_carp(ctx, ..., n_iter=1, n_strings=1): one TVS step on the common image the iteration
+    starts from (the same image, hence the same step, on every rank), then the string's DROP sweep without further
+    steps -- the placement of the single-GPU pct_iterate_carp.  With tvs=False (the default) the sweep is pct_iterate
+    and the context's TVS must be off; a context with TVS on would take a step before every block of its string."""
     address, n_slots = pct.pct_image_storage(ctx)
     x = torch.as_tensor(_DeviceArray(address, n_slots), device="cuda")
     stream = torch.cuda.current_stream() if ctx_stream is None else torch.cuda.ExternalStream(int(ctx_stream))
+    if tvs:
+        def sweep():
+            pct.pct_iterate_carp(ctx, lam, block_size, 1, 1)
+    else:
+        def sweep():
+            pct.pct_iterate(ctx, lam, block_size, 1)
     with torch.cuda.stream(stream):
-        carp_distributed(lambda: pct.pct_iterate(ctx, lam, block_size, 1), lambda: x, lambda t: None, n_iter, world)
+        carp_distributed(sweep, lambda: x, lambda t: None, n_iter, world)

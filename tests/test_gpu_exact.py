@@ -132,3 +132,46 @@ def test_runs_in_the_exact_mode(exact_oracle):
         assert np.abs(g - x_ref).max() <= 1e-3
     finally:
         pct.pct_destroy(ctx)
+
+
+def test_a_row_that_outgrows_the_scratch_is_reported_not_dropped_silently():
+    """A lane's part of the scratch holds 8 runs per segment of the longest chunk + 8 (16 on a 24-wide grid).  A history
+    at a slope no tracker delivers (dt/du = 15 at 45 degrees to the grid: each of its two segments crosses 17 voxel faces)
+    produces more.  Its row is left out of the block -- and every call that hands out results says so: pct_synchronize,
+    pct_get_image and pct_get_stats return PCT_EINTERNAL; the sane histories alone give PCT_OK."""
+    import torch
+
+    import paper_1707_05014_b200 as pct
+
+    base = synth.config(0)
+    n = 64
+    cfg = synth.Config(7, "small", n, 24, 24, 4, 1.0, 8, n, 0.1, 1, base.shapes * 0.375, seed=5)
+    H = synth.generate_numpy(cfg, n)
+    M = cfg.n_voxels
+    out = torch.zeros(M, dtype=torch.float32, device="cuda")
+    codes = []
+    for steep in (True, False):
+        Hs = {k: np.array(v, copy=True) for k, v in H.items()}
+        if steep:  # one straight line through the centre of the object, fifteen voxels sideways per voxel of depth
+            Hs["tht_in"][5] = Hs["tht_out"][5] = 15.0
+            Hs["t_in"][5], Hs["t_out"][5] = 15.0 * cfg.u_in, 15.0 * cfg.u_out
+            Hs["thv_in"][5] = Hs["thv_out"][5] = 0.0
+            Hs["v_in"][5] = Hs["v_out"][5] = 0.3
+            Hs["proj"][5] = 1  # 45 degrees (8 angles)
+        ctx = pct.pct_create(cfg.nx, cfg.ny, cfg.nz, cfg.h, cfg.u_in, cfg.u_out, torch.cuda.current_stream().cuda_stream)
+        try:
+            pct.pct_set_histories(ctx, n, to_device(Hs))
+            pct.pct_set_walk(ctx, pct.PCT_WALK_EXACT)
+            pct.pct_iterate(ctx, 0.5, n, 1)
+            got = []
+            for call in (lambda: pct.pct_synchronize(ctx), lambda: pct.pct_get_image(ctx, out, M), lambda: pct.pct_get_stats(ctx)):
+                try:
+                    call()
+                    got.append(0)
+                except pct.PctError as e:
+                    got.append(e.code)
+                    assert "more runs" in str(e)
+            codes.append(got)
+        finally:
+            pct.pct_destroy(ctx)
+    assert codes == [[-5, -5, -5], [0, 0, 0]], codes

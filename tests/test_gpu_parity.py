@@ -107,6 +107,38 @@ def test_rows_bit_exact_odd_geometry(oracle_mod, pct, torch_cuda):
     assert _check_rows(oracle_mod, pct, torch_cuda, cfg, H) > 1500
 
 
+def test_projection_index_past_the_tables_is_the_last_angle(oracle_mod, pct, torch_cuda):
+    """DESIGN.md R24 / include/pct.h pct_set_histories: "a proj[i] >= n_proj is clamped to n_proj-1".  Every third history
+    carries an index past the angle tables (n_proj, n_proj + 5, 65535): rows bit-exact and a DROP block against the oracle,
+    which reads the same rule (pinned on the CPU in test_oracle_drop.py)."""
+    cfg = synth.config(0)
+    H = synth.generate_numpy(cfg, 3000)
+    n_proj = H["proj_cos"].shape[0]
+    H["proj"] = H["proj"].copy()
+    sel = np.arange(0, 3000, 3)
+    H["proj"][sel] = np.array([n_proj, n_proj + 5, 65535], dtype=np.uint16)[np.arange(sel.size) % 3]
+    assert _check_rows(oracle_mod, pct, torch_cuda, cfg, H) > 2000
+    stats = _block_parity(oracle_mod, pct, torch_cuda, cfg, H, 0, 3000, synth.rsp_volume(cfg) * 0.9)
+    assert stats[0] > 2000
+
+
+def test_rule_reciprocal_and_square_root_are_ieee_on_every_argument_in_range(pct, torch_cuda):
+    """Bit-exactness against the CPU side rests on the rule's 1/det and sqrt(squared length) -- hardware approximation +
+    one FMA Newton step (pct_rule.cuh) -- being the correctly rounded IEEE results the oracle gets from gcc's division
+    and sqrtf.  Swept in full, not sampled: every fp32 bit pattern of the ranges DESIGN.md states for the two arguments
+    (det 1e-16 .. 1e19; squared segment length from 8e-7 mm^2 up, here to the largest finite float) and, beyond them, of
+    [2^-100, 2^100] for the reciprocal: 1.0e9 + 1.2e9 + 1.7e9 arguments, zero mismatches."""
+    bits = lambda v: int(np.float32(v).view(np.uint32))
+    s = torch_cuda.cuda.current_stream().cuda_stream
+    for which, lo, hi in ((0, 1e-16, 1e19), (1, 8e-7, np.finfo(np.float32).max), (0, 2.0 ** -100, 2.0 ** 100)):
+        assert hi > lo and bits(hi) - bits(lo) > 5e8
+        bad, first = pct.pct_debug_rule_sweep(which, bits(lo), bits(hi), s)
+        assert bad == 0, (which, bad, hex(first))
+    # the check can fail: outside the stated range the shortcut is NOT exact (the reciprocal of a huge argument is denormal, flushed to zero)
+    bad, first = pct.pct_debug_rule_sweep(0, bits(2.0 ** 126), bits(2.0 ** 127), s)
+    assert bad > 0 and first >= bits(2.0 ** 126)
+
+
 def test_rows_handcrafted_edge_cases(oracle_mod, pct, torch_cuda):
     """Misses, grazing rays, NaN, paths leaving the grid in z (dropped segments break runs),
     exactly axis-aligned central rays, steep rays."""
@@ -241,7 +273,7 @@ def test_config1_sample(oracle_mod, pct, torch_cuda):
     _run_parity(oracle_mod, pct, torch_cuda, cfg, H, cfg.lam, cfg.block_size, 2)
 
 
-def _carp_parity(oracle, pct, torch, cfg, H, lam, block, n_iter, n_strings, x0=None):
+def _carp_parity(oracle, pct, torch, cfg, H, lam, block, n_iter, n_strings, x0=None, order=None):
     """CARP run (R27-R29), image compared with the oracle after every iteration."""
     geom = oracle_geom(oracle, cfg)
     hs = oracle.Histories(H)
@@ -251,6 +283,8 @@ def _carp_parity(oracle, pct, torch, cfg, H, lam, block, n_iter, n_strings, x0=N
     ctx = _ctx(pct, torch, cfg)
     out = torch.zeros(M, dtype=torch.float32, device="cuda")
     try:
+        if order is not None:
+            pct.pct_set_option(ctx, pct.PCT_OPT_ORDER, order)
         pct.pct_set_histories(ctx, hs.n, D)
         if x0 is not None:
             pct.pct_set_image(ctx, x0.astype(np.float32), M)
@@ -293,14 +327,13 @@ def test_carp_strings_long_enough_for_the_graph_loop(oracle_mod, pct, torch_cuda
     assert np.linalg.norm(x_ref) > 1.0
 
 
-@pytest.mark.parametrize("order", ["1", "2"])
-def test_carp_config1_sample_from_an_image(oracle_mod, pct, torch_cuda, monkeypatch, order):
+@pytest.mark.parametrize("order", [1, 2])
+def test_carp_config1_sample_from_an_image(oracle_mod, pct, torch_cuda, order):
     """configs[1] geometry and block size, 3 strings of 1e5 histories, two iterations from a non-trivial image;
-    order = "2" forces the depth-slab ordering of every string's blocks."""
-    monkeypatch.setenv("PCT_ORDER", order)
+    order = 2 (pct_set_option PCT_OPT_ORDER) forces the depth-slab ordering of every string's blocks."""
     cfg = synth.config(1)
     H = synth.generate_numpy(cfg, 300_000)
-    _carp_parity(oracle_mod, pct, torch_cuda, cfg, H, cfg.lam, cfg.block_size, 2, 3, x0=synth.rsp_volume(cfg) * 0.8)
+    _carp_parity(oracle_mod, pct, torch_cuda, cfg, H, cfg.lam, cfg.block_size, 2, 3, x0=synth.rsp_volume(cfg) * 0.8, order=order)
 
 
 def test_carp_one_string_is_drop_and_arguments(pct, torch_cuda):
@@ -508,18 +541,16 @@ def test_host_entry_point_matches_device_entry_point(oracle_mod, pct, torch_cuda
     assert np.linalg.norm(imgs[0] - imgs[1]) <= 1e-5 * np.linalg.norm(imgs[0])
 
 
-@pytest.mark.parametrize("order", ["1", "2"])
-def test_pipelined_host_upload_spans_several_chunks(pct, torch_cuda, monkeypatch, order):
+@pytest.mark.parametrize("order", [1, 2])
+def test_pipelined_host_upload_spans_several_chunks(pct, torch_cuda, order):
     """pct_set_histories_host uploads in chunks of 2^20 .. 2^24 histories on a copy stream and the first
     sweep starts before the upload has finished: 9.5e6 histories (five chunks, the last one ragged) from
     pinned host arrays must give the image the device entry point gives -- for the first sweep, after
     the host arrays are overwritten once pct_synchronize has returned, for the inspection entry point
-    on the last chunk, and for a SECOND set of the same size, which reuses the device block.  order = "2"
-    forces the depth-slab ordering of the DROP blocks (by default only grids larger than the L2 get it), whose
+    on the last chunk, and for a SECOND set of the same size, which reuses the device block.  order = 2
+    (pct_set_option PCT_OPT_ORDER) forces the depth-slab ordering of the DROP blocks (by default only grids larger than the L2 get it), whose
     sort then runs batch by batch behind the upload."""
     import synth.cuda_gen as cuda_gen
-
-    monkeypatch.setenv("PCT_ORDER", order)
 
     torch = torch_cuda
     cfg = synth.config(0)
@@ -531,6 +562,7 @@ def test_pipelined_host_upload_spans_several_chunks(pct, torch_cuda, monkeypatch
     for use_host in (False, True):
         ctx = _ctx(pct, torch, cfg)
         try:
+            pct.pct_set_option(ctx, pct.PCT_OPT_ORDER, order)
             for D in sets:
                 if use_host:
                     host = {k: torch.empty(v.shape, dtype=v.dtype, pin_memory=True).copy_(v) for k, v in D.items()}
@@ -633,6 +665,61 @@ def test_carp_across_two_contexts_averaged_in_place_is_carp_with_two_strings(ora
     assert np.abs(got - x_ref).max() <= ABS_FINAL
 
 
+def test_carp_across_contexts_with_tvs_takes_one_step_per_iteration(oracle_mod, pct, torch_cuda):
+    """TVS in the one-string-per-rank form of CARP (replicas.carp_distributed_pct(tvs=True)): PAPER.md:113 puts the step
+    "just once to the initial solution at the start of each iteration", so every rank takes ONE step on the common image
+    and then sweeps its string without further steps -- pct_iterate_carp with one string.  At world = 1 through
+    carp_distributed_pct itself, and with two ranks played by two contexts of this process (as in the test above), against
+    the oracle's CARP with a TVS step per iteration and P = 1 / 2 strings."""
+    from oracle import tvs
+
+    from paper_1707_05014_b200 import replicas
+
+    torch = torch_cuda
+    cfg = synth.config(0)
+    n, B, lam, iters = 24_000, 1000, 0.5, 3
+    beta0, gamma, levels = 0.4, 0.9, 4
+    H = synth.generate_numpy(cfg, n)
+    D = to_device(H)
+    M = cfg.n_voxels
+    geom = oracle_geom(oracle_mod, cfg)
+    hs = oracle_mod.Histories(H)
+    tables = ("proj_cos", "proj_sin")
+    out = torch.zeros(M, dtype=torch.float32, device="cuda")
+    for world in (1, 2):
+        ctxs, xs = [], []
+        try:
+            for r in range(world):
+                lo, hi = replicas.string_range(r, world, n)
+                Dr = {k: (v if k in tables else v[lo:hi]) for k, v in D.items()}
+                c = _ctx(pct, torch, cfg)
+                ctxs.append((c, Dr))
+                pct.pct_set_histories(c, hi - lo, Dr)
+                pct.pct_set_tvs(c, beta0, gamma, levels)
+                addr, n_slots = pct.pct_image_storage(c)
+                xs.append(torch.as_tensor(replicas._DeviceArray(addr, n_slots), device="cuda"))
+            if world == 1:
+                replicas.carp_distributed_pct(pct, ctxs[0][0], M, lam, B, iters, 1, tvs=True)
+            else:
+                for _ in range(iters):
+                    for c, _d in ctxs:
+                        pct.pct_iterate_carp(c, lam, B, 1, 1)  # the sweep carp_distributed_pct(tvs=True) runs on a rank
+                    mean = (xs[0] + xs[1]) / 2
+                    xs[0].copy_(mean)
+                    xs[1].copy_(mean)
+            pct.pct_get_image(ctxs[-1][0], out, M)
+            got = out.cpu().numpy().astype(np.float64)
+            states = [pct.pct_get_tvs_state(c) for c, _d in ctxs]
+        finally:
+            for c, _d in ctxs:
+                pct.pct_destroy(c)
+        x_ref, beta, infos = tvs.carp_iterate_tvs(oracle_mod, geom, hs, lam, B, iters, world, np.zeros(M), beta0, gamma, levels)
+        assert np.linalg.norm(got - x_ref) <= REL_L2_PER_ITER * np.linalg.norm(x_ref), world
+        for st in states:  # one step per iteration on every rank, the same one
+            assert st["steps"] == iters and st["level"] == infos[-1]["level"]
+            assert st["beta"] == pytest.approx(beta, rel=1e-5)
+
+
 @pytest.mark.parametrize("n_strings", [2, 3])
 def test_carp_on_an_odd_grid(oracle_mod, pct, torch_cuda, n_strings):
     """CARP with several strings on the 45 x 71 x 5 grid (15975 voxels: not a multiple of four; the strings' images and
@@ -645,11 +732,10 @@ def test_carp_on_an_odd_grid(oracle_mod, pct, torch_cuda, n_strings):
 
 
 @pytest.mark.parametrize("index,n", [(0, 6001), (3, 2500), (4, 1001)])
-def test_rows_of_the_pair_walk_bit_exact(oracle_mod, pct, torch_cuda, monkeypatch, index, n):
+def test_rows_of_the_pair_walk_bit_exact(oracle_mod, pct, torch_cuda, index, n):
     """The walk of the throughput kernel (k_drop_pair: two histories per warp, sixteen lanes each, one chunk size per
-    pair) inspected directly: PCT_ROWS_PAIR=1 makes pct_debug_rows walk histories (2w, 2w+1) side by side with that code.
+    pair) inspected directly: pct_set_option(PCT_OPT_ROWS_PAIR, 1) makes pct_debug_rows walk histories (2w, 2w+1) side by side with that code.
     Voxel sequences, segment lengths (bitwise) and merged rows against the oracle; odd counts leave a lone last history."""
-    monkeypatch.setenv("PCT_ROWS_PAIR", "1")
     torch = torch_cuda
     cfg = synth.config(index)
     H = synth.generate_numpy(cfg, n)
@@ -659,6 +745,11 @@ def test_rows_of_the_pair_walk_bit_exact(oracle_mod, pct, torch_cuda, monkeypatc
     ms = geom.nmin + 2
     ctx = _ctx(pct, torch, cfg)
     try:
+        pct.pct_set_option(ctx, pct.PCT_OPT_ROWS_PAIR, 1)
+        with pytest.raises(pct.PctError):
+            pct.pct_set_option(ctx, 7, 1)
+        with pytest.raises(pct.PctError):
+            pct.pct_set_option(ctx, pct.PCT_OPT_ORDER, 3)
         pct.pct_set_histories(ctx, n, D)
         nseg = torch.zeros(n, dtype=torch.int32, device="cuda")
         nnz = torch.zeros(n, dtype=torch.int32, device="cuda")

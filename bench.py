@@ -41,7 +41,7 @@ UNIT = "protons*iterations/s"
 # per history 38 B of HBM; per segment one 4 B gather, per non-zero one 8 B (Delta, c) reduction.
 OPS_PER_SEGMENT = 106
 HBM_BYTES_PER_HISTORY = 38
-SM_COUNT = 148
+SM_COUNT_B200 = 148  # only the fallback: the run asks the device (multi_processor_count)
 LANES_PER_SM = 128
 # dram__bytes_read.sum + dram__bytes_write.sum of ONE launch of the fused accumulate kernel come from the committed ncu
 # captures of THIS build, recorded in profiles/traffic.csv (file, commit, bytes per launch with ncu's cache flush and with
@@ -56,8 +56,14 @@ def ncu_traffic(config, block_size):
         with open(TRAFFIC_CSV) as f:
             for row in csv.DictReader(f):
                 if row["config:block_size"] == "%d:%d" % (config, block_size):
-                    return {"cold_bytes": float(row["cold_bytes"]), "warm_bytes": float(row["warm_bytes"]), "commit": row["commit"],
-                            "file": row["file"], "kernel": row["kernel"]}
+                    t = {"cold_bytes": float(row["cold_bytes"]), "warm_bytes": float(row["warm_bytes"]), "commit": row["commit"],
+                         "file": row["file"], "kernel": row["kernel"]}
+                    # hardware counters of the same capture (optional columns): what the kernel is limited by as ncu sees it
+                    for k in ("warp_inst_per_launch", "issue_active", "warps_active_pct", "lts_throughput_pct", "l1_data_pipe_pct",
+                              "dram_throughput_pct", "fma_pipe_pct", "registers"):
+                        if row.get(k) not in (None, ""):
+                            t[k] = float(row[k])
+                    return t
     except (OSError, ValueError, KeyError):
         pass
     return None
@@ -73,6 +79,8 @@ def parse_args():
     ap.add_argument("--histories", type=float, default=None, help="override N (debugging only; reported)")
     ap.add_argument("--e2e-steps", type=int, default=2)
     ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--no-full", dest="full", action="store_false",
+                    help="skip the whole reconstruction (the config's own iteration count from x0 = 0, `full_reconstruction` in the line)")
     ap.add_argument("--no-cpu", action="store_true")
     ap.add_argument("--carp", action="store_true",
                     help="CARP across the ranks (the paper's own multi-processor scheme, PAPER.md:52-56): one string per rank, one "
@@ -306,6 +314,17 @@ def run_ours(args):
             out["image_finite"] = bool(torch.isfinite(img).all().item())
             out["image_mean_central"] = float(img.view(cfg.nz, cfg.ny, cfg.nx)[cfg.nz // 2, cfg.ny // 2 - 8:cfg.ny // 2 + 8,
                                                                            cfg.nx // 2 - 8:cfg.nx // 2 + 8].mean().item())
+            out["sm_count"] = torch.cuda.get_device_properties(local).multi_processor_count
+            if args.full and rank == 0:
+                # the reconstruction north_star names: the config's own iteration count from x0 = 0, histories resident
+                pct.pct_set_image(ctx, torch.zeros(M, dtype=torch.float32, device="cuda"), M)
+                pct.pct_synchronize(ctx)
+                e0.record()
+                pct.pct_iterate(ctx, lam, B, cfg.n_iter)
+                e1.record()
+                pct.pct_get_image(ctx, img, M)
+                out["full"] = {"iterations": cfg.n_iter, "seconds": e0.elapsed_time(e1) * 1e-3,
+                               "image_finite": bool(torch.isfinite(img).all().item())}
         finally:
             pct.pct_destroy(ctx)
 
@@ -348,6 +367,14 @@ def run_ours(args):
                 torch.cuda.synchronize()
                 barrier()
                 ms = max_over_ranks(e0.elapsed_time(e1))
+                if "full" in out:  # the same reconstruction end to end: pinned host histories in, host image out
+                    pct.pct_set_image(ctx, torch.zeros(M, dtype=torch.float32, device="cuda"), M)
+                    pct.pct_synchronize(ctx)
+                    t0 = time.perf_counter()
+                    pct.pct_set_histories_host(ctx, n, host)
+                    pct.pct_iterate(ctx, lam, B, cfg.n_iter)
+                    pct.pct_get_image(ctx, img_host, M)
+                    out["full"]["e2e_seconds"] = time.perf_counter() - t0
                 out["e2e"] = {"value": world * n * args.e2e_steps / (ms * 1e-3), "unit": UNIT, "h2d_bytes_per_step": h2d,
                               "d2h_bytes_per_step": 4 * M, "steps": args.e2e_steps, "ms_per_step": ms / args.e2e_steps,
                               "host_ms_per_step": {"set_histories_host": host_ms[0] / args.e2e_steps,
@@ -382,14 +409,15 @@ def run_ours(args):
     k_ms = prof["accumulate_ms"] / prof["blocks"]  # average device time of one launch
     hist_per_launch = n / prof["blocks"]
     ops = OPS_PER_SEGMENT * seg_per_hist * hist_per_launch
-    alu_peak = SM_COUNT * LANES_PER_SM * peaks["sm_max_mhz"] * 1e6 / 1e12  # T thread-instructions/s
+    sm_count = out.get("sm_count", SM_COUNT_B200)
+    alu_peak = sm_count * LANES_PER_SM * peaks["sm_max_mhz"] * 1e6 / 1e12  # T thread-instructions/s
     alu_ach = ops / (k_ms * 1e-3) / 1e12
     hbm_ach = HBM_BYTES_PER_HISTORY * hist_per_launch / (k_ms * 1e-3) / 1e9
     l2_bytes = (4.0 * seg_per_hist + 8.0 * nnz_per_hist) * hist_per_launch
     traffic = ncu_traffic(args.config, B) or {}
     t_kernel = k_ms * 1e-3
     alu = {"achieved": alu_ach, "peak": alu_peak, "unit": "Tinst/s", "frac": alu_ach / alu_peak,
-           "peak_source": "148 SM x 128 fp32 lanes x %.0f MHz (MEASURED_PEAKS.json sm_max_mhz, %s)" % (peaks["sm_max_mhz"], peaks["source"]),
+           "peak_source": "%d SM (asked of the device) x 128 fp32 lanes x %.0f MHz (MEASURED_PEAKS.json sm_max_mhz, %s)" % (sm_count, peaks["sm_max_mhz"], peaks["source"]),
            "algorithmic": "%d fp32/int ops per path segment (DESIGN.md Roofline) x %.1f segments/history x %d histories/launch" % (
                OPS_PER_SEGMENT, seg_per_hist, hist_per_launch),
            "time_at_peak_us": ops / (alu_peak * 1e12) * 1e6}
@@ -407,6 +435,21 @@ def run_ours(args):
                           "--cache-control none (warm)" % (traffic.get("file"), traffic.get("commit")) if traffic else None,
         "alu": alu, "hbm": hbm,
     }
+    issue = None
+    if "issue_active" in traffic:
+        issue = {"warp_inst_per_history": traffic["warp_inst_per_launch"] / hist_per_launch if "warp_inst_per_launch" in traffic else None,
+                 "issue_active": traffic["issue_active"], "warps_active_pct": traffic.get("warps_active_pct"),
+                 "lts_throughput_pct": traffic.get("lts_throughput_pct"), "l1_data_pipe_pct": traffic.get("l1_data_pipe_pct"),
+                 "dram_throughput_pct": traffic.get("dram_throughput_pct"), "fma_pipe_pct": traffic.get("fma_pipe_pct"),
+                 "registers_per_thread": traffic.get("registers"),
+                 "source": "%s (commit %s): one launch under ncu --set full" % (traffic.get("file"), traffic.get("commit"))}
+        # what binds, as the hardware counters see it: a memory level counts as the limiter from 60 % of its peak throughput
+        levels = {"l2": traffic.get("lts_throughput_pct", 0.0), "hbm": traffic.get("dram_throughput_pct", 0.0),
+                  "l1 data pipe": traffic.get("l1_data_pipe_pct", 0.0)}
+        top = max(levels, key=levels.get)
+        issue["binds"] = top if levels[top] >= 60.0 else (
+            "instruction issue and latency (issue slots %.0f %% busy at %.0f %% of the warp slots; no memory level above 60 %% of its "
+            "peak: %s %.0f %%)" % (100 * traffic["issue_active"], traffic.get("warps_active_pct", 0.0), top, levels[top]))
     if "peaks_l2" in out:
         pk, pw = out["peaks_l2"], out["peaks_ws"]
         rg, rr, rm = pk["gather_path_tiled_per_s"], pk["red_v2_path_tiled_per_s"], pk["mixed_pairs_tiled_per_s"]
@@ -432,7 +475,9 @@ def run_ours(args):
                            "together, %.0f G gathers/s, %.0f G reductions/s alone; peak = the same bytes at the pair rate" % (
                                rm / 1e9, rg / 1e9, rr / 1e9),
             "frac_with_rates_added_up": (t_peak_sum * hist_per_launch) / t_kernel,
-            "binds": max(times, key=times.get), "time_at_peak_us": times,
+            "binds": issue["binds"] if issue else "unknown (no ncu counters recorded for this config in profiles/traffic.csv); "
+                                                  "longest time-at-peak: " + max(times, key=times.get),
+            "time_at_peak_us": times, "issue": issue,
             "l2_rates_on_working_set": {"footprint_bytes": pw["footprint_bytes"],
                                         "gather_path_tiled_per_s": pw["gather_path_tiled_per_s"],
                                         "red_v2_path_tiled_per_s": pw["red_v2_path_tiled_per_s"],
@@ -467,6 +512,11 @@ def run_ours(args):
     if args.tvs > 0:
         line["config"]["tvs"] = "a TVS step before every block (side measurement): beta0 %g, gamma 1, 4 halvings" % args.tvs
         line["tvs"] = {"us_per_step": 1e3 * out["prof"]["tvs_ms"] / max(1, out["prof"]["blocks"]), "state": out["tvs_state"]}
+    if "full" in out:
+        line["full_reconstruction"] = dict(out["full"], workload=cfg.workload,
+                                           note="DROP, %d iterations from x0 = 0 on one B200; e2e_seconds = host clock from pinned host "
+                                                "histories to the host image.  Context only: PAPER.md:94 reports 91:43 for 0.527e9 histories "
+                                                "on 1 core + 1 Tesla (CARP, whole program, iteration count unstated)" % cfg.n_iter)
     if "e2e" in out:
         line["e2e"] = out["e2e"]
     if cpu is not None:

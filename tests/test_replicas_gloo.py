@@ -76,7 +76,7 @@ def test_world_one_needs_no_process_group():
         replicas.shard_first(-1, 10)
 
 
-def _carp_worker(rank, world, port, out_dir):
+def _carp_worker(rank, world, port, out_dir, alias=False):
     import torch
     import torch.distributed as dist
 
@@ -101,22 +101,37 @@ def _carp_worker(rank, world, port, out_dir):
         def sweep():  # the rank's local solver stands in for libpct on a GPU: one DROP sweep over its string
             state["x"], _ = oracle.drop_iterate(geom, hs, lam, B, 1, state["x"])
 
-        replicas.carp_distributed(sweep, lambda: torch.from_numpy(state["x"].copy()),
-                                  lambda t: state.update(x=t.numpy().copy()), n_iter, world)
+        if alias:
+            # the form carp_distributed_pct uses on a GPU: get_image hands out the LIVE buffer the solver works on (the
+            # library's own image array), the all-reduce and the division happen in place on it, set_image has nothing to do
+            live = torch.zeros(cfg.n_voxels, dtype=torch.float64)
+
+            def sweep_live():
+                x, _ = oracle.drop_iterate(geom, hs, lam, B, 1, live.numpy())
+                live.copy_(torch.from_numpy(x))
+
+            replicas.carp_distributed(sweep_live, lambda: live, lambda t: None, n_iter, world)
+            state["x"] = live.numpy().copy()
+        else:
+            replicas.carp_distributed(sweep, lambda: torch.from_numpy(state["x"].copy()),
+                                      lambda t: state.update(x=t.numpy().copy()), n_iter, world)
         np.save(os.path.join(out_dir, "carp_%d.npy" % rank), state["x"])
     finally:
         dist.destroy_process_group()
 
 
-def test_carp_one_string_per_rank_equals_the_single_process_definition(tmp_path):
+@pytest.mark.parametrize("alias", [False, True])
+def test_carp_one_string_per_rank_equals_the_single_process_definition(tmp_path, alias):
     """CARP with one string per rank and an all-reduce of the image per iteration (the paper's cluster form,
-    PAPER.md:52-56) gives, on every rank, what the oracle's single-process CARP gives for P = world strings."""
+    PAPER.md:52-56) gives, on every rank, what the oracle's single-process CARP gives for P = world strings -- in the copy
+    form (get_image / set_image move copies) and in the in-place alias form replicas.carp_distributed_pct uses (get_image
+    returns the live buffer, the collective works on it, set_image is a no-op)."""
     sys.path.insert(0, ROOT)
     import oracle
     import synth
 
     world, port = 2, _free_port()
-    mp.spawn(_carp_worker, args=(world, port, str(tmp_path)), nprocs=world, join=True)
+    mp.spawn(_carp_worker, args=(world, port, str(tmp_path), alias), nprocs=world, join=True)
     cfg = synth.config(0)
     H = synth.generate_numpy(cfg, 6001)
     geom = oracle.Geometry(cfg.nx, cfg.ny, cfg.nz, cfg.h, cfg.u_in, cfg.u_out)

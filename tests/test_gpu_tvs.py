@@ -13,6 +13,13 @@ from oracle import tvs
 
 pytestmark = pytest.mark.gpu
 
+# Four consecutive steps on 256 x 256 x 128 against an oracle chain that is NEVER restarted from the library's image: the
+# accepted levels agree step by step and the images stay within this relative L2 distance (measured on B200: 3.3e-8, 4.1e-8,
+# 5.0e-8, 7.3e-8 after steps 1..4).  So the chain does hold as a chain; what the per-step comparison below restarts the
+# oracle for is only its PER-VOXEL bound (1e-5 absolute), which a handful of the 8.4e6 voxels miss once the image has become
+# locally flat around them (R31's eps = 1e-6 leaves d/|d| ill-conditioned there; see the comment in the loop).
+CHAIN_DRIFT = 1e-6
+
 
 def _ctx(pct, torch, nx, ny, nz, h=1.0):
     r = 0.5 * h * min(nx, ny)
@@ -45,6 +52,8 @@ def test_single_steps_against_the_oracle(shape, beta, levels):
         xr = x.astype(np.float64)
         b = beta
         accepted = 0
+        chain = M > 1_000_000  # full size: the oracle is ALSO followed as an unbroken chain of four steps (see below)
+        xc, bc, drift = x.astype(np.float64), beta, []
         for step in range(4):
             pct.pct_tvs_step(ctx)
             pct.pct_get_image(ctx, out, M)
@@ -68,6 +77,14 @@ def test_single_steps_against_the_oracle(shape, beta, levels):
             # |d| reaches 1e-5 at some of 8.4e6 voxels, and the fp32 rounding of x, 6e-8, turns it by 1e-3): on the full-size
             # grid every step is compared on its own, the oracle restarting from the library's image.
             xr, b = (g if M > 1_000_000 else xr_new), 0.7 * info["beta_used"]
+            if chain:  # the chain never sees the library's image: decisions equal, drift bounded (CHAIN_DRIFT)
+                xc, ic = tvs.tvs_step(xc, shape, bc, levels)
+                bc = 0.7 * ic["beta_used"]
+                assert ic["level"] == st["level"], (step, ic["level"], st)
+                drift.append(float(np.linalg.norm(g - xc) / np.linalg.norm(xc)))
+        if chain:
+            print("TVS chain drift per step (rel L2, library vs unbroken oracle chain):", drift)
+            assert max(drift) <= CHAIN_DRIFT, drift
         assert accepted >= 2 and st["accepted"] == accepted
         pct.pct_set_tvs(ctx, 0.0, 1.0, 1)  # off again
         with pytest.raises(pct.PctError):
